@@ -1,0 +1,151 @@
+/*
+ * rs.h -- C ABI of librs: batched Kohn-Sham  H psi = -1/2 Lap psi + V_loc psi  on a real-space mesh,
+ * applied to a BLOCK of orbitals at once (arxiv:1306.2953; citations are /root/reference/PAPER.md
+ * line + section).  Hand-written CUDA for sm_100a behind plain pointers; no torch types here.
+ *
+ * The problem, as the paper states it
+ *   - H = -1/2 Lap + v(r), applied as an operator, never stored (PAPER.md:41 eq. 2; :119 sec. V).
+ *   - The mesh is a uniform lattice of spacing h restricted to the union of spheres of radius R
+ *     around the atoms (PAPER.md:53 sec. II; :354 sec. XII).  psi = 0 outside (reading S3).
+ *   - Lap is a high-order finite-difference star: half-width n ("order"), 6n+1 points; the
+ *     paper's "fourth-order ... stencil size of 25" is n = 4 (sec. V.A).
+ *   - Routines receive a GROUP of orbitals (sec. IV); the block is stored with the
+ *     orbital index fastest: element (point ip, orbital j) at  ip*B + j  (Fig. 4 :107).
+ *     The block size B is a run-time power of two.
+ *   - All local potentials are pre-summed into one array (sec. V.B).
+ *   - Neighbours are found through a table because the shape is arbitrary.
+ *
+ * Conventions
+ *   - "host"/"dev" on every pointer says where the memory lives.  The caller owns every buffer it
+ *     passes; the mesh handle owns its own host tables and device tables.
+ *   - Mesh order: the library chooses the enumeration of the np in-domain points (brick order, see
+ *     DESIGN.md); rs_mesh_get_points() publishes it.  Every per-point array (vloc, states, block
+ *     rows) is indexed by that order.
+ *   - Block layout: [nrows][ldb] elements, nrows = np + 1, ldb = B.  Row np is the ZERO SLOT: pack
+ *     writes zeros there, apply never writes it, and apply REQUIRES it to be zero in psi.  Columns
+ *     j >= nst_in_block are zero after pack and are ignored by unpack.
+ *   - dtype RS_REAL64: element = double.  RS_COMPLEX128: element = interleaved (re, im) doubles; the
+ *     weights and V are real, so a complex block of width B is computed as 2B independent real columns.
+ *   - rs_block_pack / rs_block_unpack / rs_hamiltonian_apply are asynchronous on `stream`
+ *     (a cudaStream_t passed as void*; NULL = legacy default stream), allocate nothing and never
+ *     synchronise.  The first use of a given fd_order on a mesh uploads that order's neighbour table
+ *     (one synchronous cudaMalloc + copy, then cached in the handle).
+ *   - Every function returns rs_status; nothing throws.  rs_last_error() gives thread-local text for
+ *     the last non-OK status.  There is no CPU fallback: without a CUDA device the compute entry
+ *     points return RS_ERR_CUDA.
+ */
+#ifndef RS_H
+#define RS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rs_mesh rs_mesh; /* opaque */
+
+typedef enum {
+    RS_OK = 0,
+    RS_ERR_INVALID_ARG = 1,
+    RS_ERR_ALLOC = 2,
+    RS_ERR_CUDA = 3,
+    RS_ERR_UNSUPPORTED = 4
+} rs_status;
+
+typedef enum { RS_REAL64 = 0, RS_COMPLEX128 = 1 } rs_dtype;
+
+/* Point enumeration (sec. V.A, Fig. 7: "enumerate the grid points based on a
+ * sequence of small parallelepipedic grids").  Results do not depend on it beyond rounding order. */
+typedef enum {
+    RS_ORDER_BRICK = 0, /* 4x4x4 bricks, brick after brick (default; enables the brick kernel) */
+    RS_ORDER_LEX = 1    /* lexicographic (i, j, k), k fastest: the paper's "standard order"    */
+} rs_ordering;
+
+/* Kernel selection for rs_hamiltonian_apply_v (tests and ablations; results agree to rounding). */
+typedef enum {
+    RS_KERNEL_AUTO = 0,   /* best available for this mesh / order / width                         */
+    RS_KERNEL_GATHER = 1, /* per-point neighbour table, one gathered load per star arm (any mesh) */
+    RS_KERNEL_BRICK = 2   /* brick-tiled shared-memory kernel (RS_ORDER_BRICK, non-periodic)      */
+} rs_kernel;
+
+#define RS_MAX_FD_ORDER 8
+#define RS_MAX_BLOCK 64
+
+/* ---- mesh (host builder; steps a1-a3 of SURVEY.md section 8(a)) ---------------------------------
+ * rs_mesh_create: enumerate the lattice points (i,j,k)*spacing, integer i,j,k, lying in the closed
+ * ball of `radius` around any of the `nc` centres (host [nc][3], bohr); choose the enumeration; build
+ * the tables; upload them.  max_fd_order bounds the fd_order later passed to apply (1..RS_MAX_FD_ORDER).
+ * Works without a CUDA device (tables stay on the host; compute calls then fail with RS_ERR_CUDA).   */
+rs_status rs_mesh_create(const double *centers_host, int nc, double radius, double spacing,
+                         int max_fd_order, rs_mesh **out);
+rs_status rs_mesh_create_ordered(const double *centers_host, int nc, double radius, double spacing,
+                                 int max_fd_order, rs_ordering ordering, rs_mesh **out);
+/* Full rectangular test mesh, lattice indices 0..n-1 per axis.  periodic = 1 wraps all three axes
+ * (then no arm ever leaves the mesh), periodic = 0 is zero-Dirichlet like the sphere meshes.        */
+rs_status rs_mesh_create_box(int nx, int ny, int nz, double spacing, int max_fd_order, int periodic,
+                             rs_ordering ordering, rs_mesh **out);
+rs_status rs_mesh_destroy(rs_mesh *mesh);
+
+int64_t rs_mesh_npoints(const rs_mesh *mesh);           /* np; -1 if mesh is NULL                   */
+double rs_mesh_spacing(const rs_mesh *mesh);
+int64_t rs_mesh_nbricks(const rs_mesh *mesh);           /* number of non-empty 4x4x4 bricks (0 for LEX) */
+/* ijk_host [np][3] int32: lattice indices of the points, in mesh order.                            */
+rs_status rs_mesh_get_points(const rs_mesh *mesh, int32_t *ijk_host);
+/* map_host [np][6*fd_order] int32: entry (ip, s) is the mesh index of the point at arm s of ip, or np
+ * (the zero slot) if that point is outside the mesh.  Arm order: s = axis*2n + 2*(k-1) + (0 for +k,
+ * 1 for -k), axis 0 = i, k = 1..n.  This is the table of PAPER.md:131 in its plain form; the brick
+ * kernel uses a compact form that expands to exactly this (reading S15).                           */
+rs_status rs_mesh_get_index_map(const rs_mesh *mesh, int fd_order, int32_t *map_host);
+
+/* Bytes of one block buffer: (np + 1) * block_size * (8 or 16).  0 on bad arguments.               */
+size_t rs_block_bytes(const rs_mesh *mesh, int block_size, rs_dtype dtype);
+
+/* ---- layout transforms (steps a4, a6; Fig. 4) ---------------------------------------
+ * states (dev): [nst_total][ld] elements, orbital-major (Fig. 4a), ld >= np, points in mesh order.
+ * pack:   block[ip*B + j] = states[(ist0 + j)*ld + ip]   for j < nst_in_block, ip < np;
+ *         zero for j >= nst_in_block and for row np.
+ * unpack: states[(ist0 + j)*ld + ip] = block[ip*B + j]   for j < nst_in_block, ip < np.
+ * block_size must be a power of two in 1..RS_MAX_BLOCK, 1 <= nst_in_block <= block_size.           */
+rs_status rs_block_pack(const rs_mesh *mesh, const void *states_dev, int64_t ld, int ist0, int nst_in_block,
+                        int block_size, void *block_dev, rs_dtype dtype, void *stream);
+rs_status rs_block_unpack(const rs_mesh *mesh, const void *block_dev, int block_size, int nst_in_block,
+                          void *states_dev, int64_t ld, int ist0, rs_dtype dtype, void *stream);
+
+/* ---- the fused stencil + local potential (step a5; eq. 2 :41) -------------
+ *   hpsi[ip][j] = -1/(2 h^2) [ 3 c_0 psi[ip][j] + sum_{m=1..n} c_m sum_{axes} (psi[ip + m e][j] + psi[ip - m e][j]) ]
+ *                 + vloc[ip] psi[ip][j],      ip < np, j < nst;   psi = 0 outside the mesh.
+ * coeffs_host: c_0..c_n, dimensionless (the library forms w_k = -0.5 c_k / h^2 in fp64, reading S6).
+ * vloc_dev: [np] doubles, mesh order.  psi_dev / hpsi_dev: block buffers of width nst (= the block
+ * size B of this call: 1, 2, 4, ..., 64), distinct and non-overlapping.  Row np of hpsi is left as is.
+ * Errors: NULL pointers, nst not a power of two in 1..64, fd_order < 1 or > max_fd_order, psi == hpsi
+ * -> RS_ERR_INVALID_ARG; launch failure or no device -> RS_ERR_CUDA.                               */
+rs_status rs_hamiltonian_apply(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
+                               const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
+                               rs_dtype dtype, void *stream);
+/* Same, with an explicit kernel choice; RS_ERR_UNSUPPORTED if that kernel cannot serve this call.  */
+rs_status rs_hamiltonian_apply_v(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
+                                 const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
+                                 rs_dtype dtype, void *stream, rs_kernel kernel);
+
+/* ---- whole path on HOST buffers (step a7: the block sweep; used for the end-to-end number) --------
+ * states_host / hstates_host: pinned or pageable host arrays [nst_total][ld] (ld >= np, mesh order);
+ * vloc_host [np].  Uploads, then for each block of `block_size` orbitals: pack, apply, unpack; then
+ * downloads H psi.  Allocates its device workspace per call and synchronises before returning.     */
+rs_status rs_hamiltonian_apply_states_host(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
+                                           const double *vloc_host, const void *states_host,
+                                           void *hstates_host, int64_t ld, int nst_total, int block_size,
+                                           rs_dtype dtype);
+
+const char *rs_last_error(void);
+/* Static description of the kernel rs_hamiltonian_apply would pick ("gather", "brick", ...).       */
+const char *rs_kernel_name(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, rs_kernel kernel);
+/* Bytes of neighbour structure the chosen kernel reads per call (for the roofline's algorithmic bytes). */
+int64_t rs_kernel_table_bytes(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, rs_kernel kernel);
+int rs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RS_H */

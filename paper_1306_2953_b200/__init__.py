@@ -1,0 +1,247 @@
+"""Thin Python binding of librs.so (include/rs.h): argument marshalling only.
+
+Every step of the path -- mesh enumeration, neighbour tables, pack/unpack, the fused stencil +
+potential -- runs inside the library (C++ host code and hand-written sm_100a CUDA kernels).  PyTorch
+appears only as the owner of device memory and streams: tensors are passed as raw pointers.
+
+There is no CPU fallback: importing this package without a loadable librs.so raises, and the
+compute calls raise RsError(RS_ERR_CUDA) when no CUDA device is present.
+
+Function names mirror the C ABI (rs_mesh_create, rs_block_pack, rs_block_unpack,
+rs_hamiltonian_apply, ...); see include/rs.h for the meaning of every argument and for the
+passages of the paper that define each operation.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import shutil
+
+import numpy as np
+
+from . import build as _build
+
+RS_OK, RS_ERR_INVALID_ARG, RS_ERR_ALLOC, RS_ERR_CUDA, RS_ERR_UNSUPPORTED = range(5)
+RS_REAL64, RS_COMPLEX128 = 0, 1
+RS_ORDER_BRICK, RS_ORDER_LEX = 0, 1
+RS_KERNEL_AUTO, RS_KERNEL_GATHER, RS_KERNEL_BRICK = 0, 1, 2
+RS_MAX_FD_ORDER = 8
+RS_MAX_BLOCK = 64
+
+_STATUS_NAMES = {0: "RS_OK", 1: "RS_ERR_INVALID_ARG", 2: "RS_ERR_ALLOC", 3: "RS_ERR_CUDA", 4: "RS_ERR_UNSUPPORTED"}
+
+# every symbol include/rs.h declares (tests check that the library exports all of them)
+EXPORTS = (
+    "rs_mesh_create", "rs_mesh_create_ordered", "rs_mesh_create_box", "rs_mesh_destroy", "rs_mesh_npoints",
+    "rs_mesh_spacing", "rs_mesh_nbricks", "rs_mesh_get_points", "rs_mesh_get_index_map", "rs_block_bytes",
+    "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
+    "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version",
+)
+
+
+class RsError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{_STATUS_NAMES.get(status, status)}: {message}")
+        self.status = status
+
+
+def _load() -> C.CDLL:
+    so = _build.SO
+    if not os.path.exists(so):
+        if shutil.which(os.environ.get("NVCC", "nvcc")) is None:
+            raise ImportError(f"{so} is missing and nvcc is not available to build it; there is no fallback path")
+        _build.build()
+    L = C.CDLL(so)
+    vp, dp, i32p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int32)
+    L.rs_mesh_create.argtypes = [dp, C.c_int, C.c_double, C.c_double, C.c_int, C.POINTER(vp)]
+    L.rs_mesh_create_ordered.argtypes = [dp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.POINTER(vp)]
+    L.rs_mesh_create_box.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.POINTER(vp)]
+    L.rs_mesh_destroy.argtypes = [vp]
+    L.rs_mesh_npoints.argtypes = [vp]
+    L.rs_mesh_npoints.restype = C.c_int64
+    L.rs_mesh_spacing.argtypes = [vp]
+    L.rs_mesh_spacing.restype = C.c_double
+    L.rs_mesh_nbricks.argtypes = [vp]
+    L.rs_mesh_nbricks.restype = C.c_int64
+    L.rs_mesh_get_points.argtypes = [vp, i32p]
+    L.rs_mesh_get_index_map.argtypes = [vp, C.c_int, i32p]
+    L.rs_block_bytes.argtypes = [vp, C.c_int, C.c_int]
+    L.rs_block_bytes.restype = C.c_size_t
+    L.rs_block_pack.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, vp, C.c_int, vp]
+    L.rs_block_unpack.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int64, C.c_int, C.c_int, vp]
+    L.rs_hamiltonian_apply.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp]
+    L.rs_hamiltonian_apply_v.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp, C.c_int]
+    L.rs_hamiltonian_apply_states_host.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int]
+    L.rs_last_error.restype = C.c_char_p
+    L.rs_kernel_name.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
+    L.rs_kernel_name.restype = C.c_char_p
+    L.rs_kernel_table_bytes.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
+    L.rs_kernel_table_bytes.restype = C.c_int64
+    L.rs_version.restype = C.c_int
+    return L
+
+
+_lib = _load()
+LIBRARY_PATH = _build.SO
+
+
+def _check(status: int) -> None:
+    if status != RS_OK:
+        raise RsError(status, (_lib.rs_last_error() or b"").decode())
+
+
+def _dptr(a: np.ndarray):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ptr(t) -> int:
+    """Raw address of a torch tensor (device or host) or a numpy array."""
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def _stream(stream) -> int:
+    """cudaStream_t as an integer: None -> torch's current stream, int -> as given, torch Stream -> its handle."""
+    if stream is None:
+        import torch
+
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _dtype_of(t) -> int:
+    s = str(t.dtype)
+    if s.endswith("float64"):
+        return RS_REAL64
+    if s.endswith("complex128"):
+        return RS_COMPLEX128
+    raise TypeError(f"unsupported element type {t.dtype}: the path computes in fp64 (real or complex)")
+
+
+class Mesh:
+    """Owner of an rs_mesh handle (host tables + device tables)."""
+
+    def __init__(self, handle: int):
+        self._h = C.c_void_p(handle)
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h and _lib is not None:
+            _lib.rs_mesh_destroy(h)
+
+    @property
+    def handle(self) -> C.c_void_p:
+        if not self._h:
+            raise RsError(RS_ERR_INVALID_ARG, "mesh already destroyed")
+        return self._h
+
+    @property
+    def npoints(self) -> int:
+        return int(_lib.rs_mesh_npoints(self.handle))
+
+    @property
+    def spacing(self) -> float:
+        return float(_lib.rs_mesh_spacing(self.handle))
+
+    @property
+    def nbricks(self) -> int:
+        return int(_lib.rs_mesh_nbricks(self.handle))
+
+    def points(self) -> np.ndarray:
+        return rs_mesh_get_points(self)
+
+    def index_map(self, fd_order: int) -> np.ndarray:
+        return rs_mesh_get_index_map(self, fd_order)
+
+
+def rs_version() -> int:
+    return int(_lib.rs_version())
+
+
+def rs_mesh_create(centers, radius: float, spacing: float, max_fd_order: int = 4,
+                   ordering: int = RS_ORDER_BRICK) -> Mesh:
+    c = np.ascontiguousarray(centers, dtype=np.float64).reshape(-1, 3)
+    out = C.c_void_p()
+    _check(_lib.rs_mesh_create_ordered(_dptr(c), c.shape[0], radius, spacing, max_fd_order, ordering, C.byref(out)))
+    return Mesh(out.value)
+
+
+def rs_mesh_create_box(nx: int, ny: int, nz: int, spacing: float, max_fd_order: int = 4, periodic: bool = False,
+                       ordering: int = RS_ORDER_BRICK) -> Mesh:
+    out = C.c_void_p()
+    _check(_lib.rs_mesh_create_box(nx, ny, nz, spacing, max_fd_order, int(periodic), ordering, C.byref(out)))
+    return Mesh(out.value)
+
+
+def rs_mesh_destroy(mesh: Mesh) -> None:
+    h, mesh._h = mesh._h, None
+    if h:
+        _check(_lib.rs_mesh_destroy(h))
+
+
+def rs_mesh_npoints(mesh: Mesh) -> int:
+    return mesh.npoints
+
+
+def rs_mesh_get_points(mesh: Mesh) -> np.ndarray:
+    ijk = np.empty((mesh.npoints, 3), dtype=np.int32)
+    _check(_lib.rs_mesh_get_points(mesh.handle, ijk.ctypes.data_as(C.POINTER(C.c_int32))))
+    return ijk
+
+
+def rs_mesh_get_index_map(mesh: Mesh, fd_order: int) -> np.ndarray:
+    m = np.empty((mesh.npoints, 6 * fd_order), dtype=np.int32)
+    _check(_lib.rs_mesh_get_index_map(mesh.handle, fd_order, m.ctypes.data_as(C.POINTER(C.c_int32))))
+    return m
+
+
+def rs_block_bytes(mesh: Mesh, block_size: int, dtype: int = RS_REAL64) -> int:
+    return int(_lib.rs_block_bytes(mesh.handle, block_size, dtype))
+
+
+def rs_block_pack(mesh: Mesh, states, ist0: int, nst_in_block: int, block_size: int, block, stream=None,
+                  ld: int | None = None) -> None:
+    """states: device tensor [nst_total][ld]; block: device tensor of rs_block_bytes() bytes."""
+    ld = int(states.shape[-1]) if ld is None else ld
+    _check(_lib.rs_block_pack(mesh.handle, _ptr(states), ld, ist0, nst_in_block, block_size, _ptr(block),
+                              _dtype_of(states), _stream(stream)))
+
+
+def rs_block_unpack(mesh: Mesh, block, block_size: int, nst_in_block: int, states, ist0: int, stream=None,
+                    ld: int | None = None) -> None:
+    ld = int(states.shape[-1]) if ld is None else ld
+    _check(_lib.rs_block_unpack(mesh.handle, _ptr(block), block_size, nst_in_block, _ptr(states), ld, ist0,
+                                _dtype_of(states), _stream(stream)))
+
+
+def rs_hamiltonian_apply(mesh: Mesh, fd_order: int, coeffs, vloc, psi, hpsi, nst: int, dtype: int | None = None,
+                         stream=None, kernel: int = RS_KERNEL_AUTO) -> None:
+    """hpsi <- -1/2 Lap psi + vloc psi on one block of width nst (device tensors); asynchronous on `stream`."""
+    c = np.ascontiguousarray(coeffs, dtype=np.float64)
+    if c.shape != (fd_order + 1,):
+        raise RsError(RS_ERR_INVALID_ARG, "coeffs must hold c_0..c_n")
+    dtype = _dtype_of(psi) if dtype is None else dtype
+    _check(_lib.rs_hamiltonian_apply_v(mesh.handle, fd_order, _dptr(c), _ptr(vloc), _ptr(psi), _ptr(hpsi), nst,
+                                       dtype, _stream(stream), kernel))
+
+
+def rs_hamiltonian_apply_states_host(mesh: Mesh, fd_order: int, coeffs, vloc_host, states_host, hstates_host,
+                                     block_size: int) -> None:
+    """Whole path on HOST arrays [nst_total][ld] (numpy or CPU torch tensors): H2D, pack/apply/unpack per block, D2H."""
+    c = np.ascontiguousarray(coeffs, dtype=np.float64)
+    nst_total, ld = int(states_host.shape[0]), int(states_host.shape[1])
+    _check(_lib.rs_hamiltonian_apply_states_host(mesh.handle, fd_order, _dptr(c), _ptr(vloc_host), _ptr(states_host),
+                                                 _ptr(hstates_host), ld, nst_total, block_size,
+                                                 _dtype_of(states_host)))
+
+
+def rs_kernel_name(mesh: Mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, kernel: int = RS_KERNEL_AUTO) -> str:
+    return _lib.rs_kernel_name(mesh.handle, fd_order, nst, dtype, kernel).decode()
+
+
+def rs_kernel_table_bytes(mesh: Mesh, fd_order: int, nst: int, dtype: int = RS_REAL64,
+                          kernel: int = RS_KERNEL_AUTO) -> int:
+    return int(_lib.rs_kernel_table_bytes(mesh.handle, fd_order, nst, dtype, kernel))

@@ -1,0 +1,144 @@
+// C-ABI entry points: argument checks, weight formation, kernel dispatch, host-buffer sweep.
+#include <cstring>
+
+#include "rs_internal.h"
+
+static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
+
+extern "C" rs_status rs_block_pack(const rs_mesh *m, const void *states, int64_t ld, int ist0, int nst_in, int B,
+                                   void *block, rs_dtype dtype, void *stream)
+{
+    if (!m || !states || !block || ld < m->np || ist0 < 0 || !pow2_in(B, 1, RS_MAX_BLOCK) || nst_in < 1 || nst_in > B ||
+        (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_block_pack: bad argument");
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    return rs_launch_pack(m, states, ld, ist0, nst_in, B, block, dtype == RS_COMPLEX128 ? 2 : 1, (cudaStream_t)stream);
+}
+
+extern "C" rs_status rs_block_unpack(const rs_mesh *m, const void *block, int B, int nst_in, void *states, int64_t ld,
+                                     int ist0, rs_dtype dtype, void *stream)
+{
+    if (!m || !states || !block || ld < m->np || ist0 < 0 || !pow2_in(B, 1, RS_MAX_BLOCK) || nst_in < 1 || nst_in > B ||
+        (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_block_unpack: bad argument");
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    return rs_launch_unpack(m, block, B, nst_in, states, ld, ist0, dtype == RS_COMPLEX128 ? 2 : 1, (cudaStream_t)stream);
+}
+
+static rs_status check_apply(const rs_mesh *m, int n, const double *coeffs, const double *vloc, const void *psi,
+                             const void *hpsi, int nst, rs_dtype dtype)
+{
+    if (!m || !coeffs || !vloc || !psi || !hpsi) return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: null argument");
+    if (n < 1 || n > m->max_n) return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: fd_order outside 1..max_fd_order");
+    if (!pow2_in(nst, 1, RS_MAX_BLOCK)) return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: nst must be 1,2,4,...,64");
+    if (dtype != RS_REAL64 && dtype != RS_COMPLEX128) return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: bad dtype");
+    const size_t bytes = rs_block_bytes(m, nst, dtype);
+    const char *a = (const char *)psi, *b = (const char *)hpsi;
+    if (a == b || (a < b + bytes && b < a + bytes))
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: psi and hpsi overlap");
+    return RS_OK;
+}
+
+static rs_kernel resolve_kernel(const rs_mesh *m, int n, int ncol, rs_kernel k)
+{
+    if (k == RS_KERNEL_AUTO) return rs_brick_supported(m, n, ncol) ? RS_KERNEL_BRICK : RS_KERNEL_GATHER;
+    return k;
+}
+
+extern "C" rs_status rs_hamiltonian_apply_v(const rs_mesh *m, int n, const double *coeffs, const double *vloc,
+                                            const void *psi, void *hpsi, int nst, rs_dtype dtype, void *stream,
+                                            rs_kernel kernel)
+{
+    rs_status st = check_apply(m, n, coeffs, vloc, psi, hpsi, nst, dtype);
+    if (st != RS_OK) return st;
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    rs_weights w;
+    std::memset(&w, 0, sizeof(w));
+    for (int k = 0; k <= n; ++k) w.w[k] = -0.5 * coeffs[k] / (m->h * m->h);
+    const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);  // complex = 2 independent real columns
+    const rs_kernel k = resolve_kernel(m, n, ncol, kernel);
+    if (k == RS_KERNEL_BRICK) {
+        if (!rs_brick_supported(m, n, ncol)) return rs_fail(RS_ERR_UNSUPPORTED, "brick kernel cannot serve this call");
+        return rs_launch_brick(m, n, w, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
+    }
+    if (k != RS_KERNEL_GATHER) return rs_fail(RS_ERR_INVALID_ARG, "unknown kernel id");
+    const int32_t *d_map = nullptr;
+    st = rs_mesh_device_map(m, n, &d_map);
+    if (st != RS_OK) return st;
+    return rs_launch_gather(m, n, w, d_map, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
+}
+
+extern "C" rs_status rs_hamiltonian_apply(const rs_mesh *m, int n, const double *coeffs, const double *vloc,
+                                          const void *psi, void *hpsi, int nst, rs_dtype dtype, void *stream)
+{
+    return rs_hamiltonian_apply_v(m, n, coeffs, vloc, psi, hpsi, nst, dtype, stream, RS_KERNEL_AUTO);
+}
+
+extern "C" const char *rs_kernel_name(const rs_mesh *m, int n, int nst, rs_dtype dtype, rs_kernel kernel)
+{
+    if (!m) return "none";
+    const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
+    return resolve_kernel(m, n, ncol, kernel) == RS_KERNEL_BRICK ? "brick" : "gather";
+}
+
+extern "C" int64_t rs_kernel_table_bytes(const rs_mesh *m, int n, int nst, rs_dtype dtype, rs_kernel kernel)
+{
+    if (!m) return 0;
+    const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
+    if (resolve_kernel(m, n, ncol, kernel) == RS_KERNEL_BRICK) return rs_brick_table_bytes(m);
+    return m->np * 6 * (int64_t)n * 4;
+}
+
+// Whole path on host buffers (a7): H2D, then per block pack -> apply -> unpack, then D2H.
+extern "C" rs_status rs_hamiltonian_apply_states_host(const rs_mesh *m, int n, const double *coeffs,
+                                                      const double *vloc_host, const void *states_host,
+                                                      void *hstates_host, int64_t ld, int nst_total, int B,
+                                                      rs_dtype dtype)
+{
+    if (!m || !coeffs || !vloc_host || !states_host || !hstates_host || ld < m->np || nst_total < 1 ||
+        !pow2_in(B, 1, RS_MAX_BLOCK) || n < 1 || n > m->max_n || (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply_states_host: bad argument");
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    const size_t esz = dtype == RS_COMPLEX128 ? 16 : 8;
+    const size_t sbytes = (size_t)nst_total * ld * esz, bbytes = rs_block_bytes(m, B, dtype);
+    void *d_states = nullptr, *d_out = nullptr, *d_psi = nullptr, *d_hpsi = nullptr;
+    double *d_v = nullptr;
+    cudaStream_t st = nullptr;
+    rs_status rc = RS_OK;
+    auto cleanup = [&]() {
+        cudaFree(d_states), cudaFree(d_out), cudaFree(d_psi), cudaFree(d_hpsi), cudaFree(d_v);
+        if (st) cudaStreamDestroy(st);
+    };
+#define TRY_OR_CLEAN(call)                                                                     \
+    do {                                                                                       \
+        cudaError_t _e = (call);                                                               \
+        if (_e != cudaSuccess) {                                                               \
+            cleanup();                                                                         \
+            return rs_fail(RS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e));   \
+        }                                                                                      \
+    } while (0)
+    TRY_OR_CLEAN(cudaStreamCreate(&st));
+    TRY_OR_CLEAN(cudaMalloc(&d_states, sbytes));
+    TRY_OR_CLEAN(cudaMalloc(&d_out, sbytes));
+    TRY_OR_CLEAN(cudaMalloc(&d_psi, bbytes));
+    TRY_OR_CLEAN(cudaMalloc(&d_hpsi, bbytes));
+    TRY_OR_CLEAN(cudaMalloc(&d_v, (size_t)m->np * 8));
+    TRY_OR_CLEAN(cudaMemcpyAsync(d_v, vloc_host, (size_t)m->np * 8, cudaMemcpyHostToDevice, st));
+    TRY_OR_CLEAN(cudaMemcpyAsync(d_states, states_host, sbytes, cudaMemcpyHostToDevice, st));
+    for (int ist0 = 0; ist0 < nst_total && rc == RS_OK; ist0 += B) {
+        const int nb = nst_total - ist0 < B ? nst_total - ist0 : B;
+        rc = rs_block_pack(m, d_states, ld, ist0, nb, B, d_psi, dtype, st);
+        if (rc == RS_OK) rc = rs_hamiltonian_apply(m, n, coeffs, d_v, d_psi, d_hpsi, B, dtype, st);
+        if (rc == RS_OK) rc = rs_block_unpack(m, d_hpsi, B, nb, d_out, ld, ist0, dtype, st);
+    }
+    if (rc != RS_OK) {
+        cudaStreamSynchronize(st);
+        cleanup();
+        return rc;
+    }
+    TRY_OR_CLEAN(cudaMemcpyAsync(hstates_host, d_out, sbytes, cudaMemcpyDeviceToHost, st));
+    TRY_OR_CLEAN(cudaStreamSynchronize(st));
+    cleanup();
+#undef TRY_OR_CLEAN
+    return RS_OK;
+}

@@ -139,3 +139,15 @@ def shard_orbitals(nst_total: int, block: int, rank: int, world: int) -> tuple[i
     lo = (nblk * rank) // world
     hi = (nblk * (rank + 1)) // world
     return min(lo * block, nst_total), min(hi * block, nst_total)
+
+
+def canonical_rank(ijk: np.ndarray) -> np.ndarray:
+    """rank[ip] = position of mesh point ip in the canonical (lexicographic i, j, k) order of the same
+    point set.  `ijk` is whatever enumeration a mesh builder publishes; orbitals generated in
+    canonical order are brought to that enumeration with  psi_mesh = psi_canon[..., rank]  and back
+    with  out_canon[..., rank] = out_mesh.  Pure index bookkeeping on inputs/outputs."""
+    ijk = np.asarray(ijk)
+    order = np.lexsort((ijk[:, 2], ijk[:, 1], ijk[:, 0]))  # canonical position -> mesh index
+    rank = np.empty(order.size, dtype=np.int64)
+    rank[order] = np.arange(order.size, dtype=np.int64)
+    return rank

@@ -1,0 +1,211 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the same seeded
+inputs, element by element (configs 0-1 and small boxes: several tiles, ragged tails, every block
+size, both enumerations, every kernel, real and complex, orders 1..8)."""
+import numpy as np
+import pytest
+
+import oracle
+import synthetic
+import paper_1306_2953_b200 as rs
+from harness import EPS, Problem, check
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = {"auto": rs.RS_KERNEL_AUTO, "gather": rs.RS_KERNEL_GATHER, "brick": rs.RS_KERNEL_BRICK}
+_cache = {}
+
+
+def problem(i, ordering=rs.RS_ORDER_BRICK):
+    key = (i, ordering)
+    if key not in _cache:
+        _cache[key] = Problem.from_config(i, ordering=ordering)
+    return _cache[key]
+
+
+def _run(p, psi, n, B, kernel):
+    try:
+        return p.gpu_hpsi(psi, n, B, kernel=KERNELS[kernel])
+    except rs.RsError as e:
+        if e.status == rs.RS_ERR_UNSUPPORTED and kernel != "auto":
+            pytest.skip(f"{kernel} kernel does not serve this call: {e}")
+        raise
+
+
+# ---- config 0: tiny atom, nst=4, B=4 (BASELINE.json configs[0]) ---------------------------------
+@pytest.mark.parametrize("kernel", ["auto", "gather", "brick"])
+@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX])
+def test_config0(kernel, ordering):
+    p = problem(0, ordering)
+    cfg = p.cfg
+    psi = synthetic.orbitals(cfg.seed, 0, cfg.nst, p.np)
+    g = _run(p, psi, 4, 4, kernel)
+    o = p.oracle_hpsi(psi, 4)
+    check(g, o, p.cond_denominator(psi, 4), "config0")
+
+
+# ---- config 1: benzene-shaped, nst=16, every block size 1..64 (padded) --------------------------
+@pytest.mark.parametrize("kernel", ["auto", "gather"])
+@pytest.mark.parametrize("B", [1, 2, 4, 8, 16, 32, 64])
+def test_config1_real(B, kernel):
+    p = problem(1)
+    cfg = p.cfg
+    psi = synthetic.orbitals(cfg.seed, 0, cfg.nst, p.np)
+    g = _run(p, psi, 4, B, kernel)
+    o = p.oracle_hpsi(psi, 4)
+    check(g, o, p.cond_denominator(psi, 4), f"config1 B={B}")
+
+
+@pytest.mark.parametrize("kernel", ["auto", "gather"])
+@pytest.mark.parametrize("B", [1, 2, 8, 32, 64])
+def test_config1_complex(B, kernel):
+    p = problem(1)
+    psi = synthetic.orbitals(31, 0, 6, p.np, is_complex=True)      # 6 orbitals: ragged last block for B=4..
+    g = _run(p, psi, 4, B, kernel)
+    o = p.oracle_hpsi(psi, 4)
+    check(g, o, p.cond_denominator(psi, 4), f"config1 complex B={B}")
+
+
+@pytest.mark.parametrize("kernel", ["auto", "gather"])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8])
+def test_other_orders(n, kernel):
+    cfg = synthetic.config(0)
+    key = ("orders", 8)
+    if key not in _cache:
+        _cache[key] = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=8)
+    p = _cache[key]
+    psi = synthetic.orbitals(5, 0, 5, p.np)
+    g = _run(p, psi, n, 4, kernel)                                  # 5 orbitals in blocks of 4: 4 + 1 (padded)
+    o = p.oracle_hpsi(psi, n)
+    check(g, o, p.cond_denominator(psi, n), f"order {n}")
+
+
+def test_config1_order6_lex_ordering():
+    p = problem(1, rs.RS_ORDER_LEX)
+    psi = synthetic.orbitals(2, 0, 3, p.np)
+    g = p.gpu_hpsi(psi, 6, 2, ld_pad=5)
+    o = p.oracle_hpsi(psi, 6)
+    check(g, o, p.cond_denominator(psi, 6), "config1 lex n=6")
+
+
+# ---- test boxes: Dirichlet and periodic, sizes that are not multiples of the brick / tile -------
+@pytest.mark.parametrize("kernel", ["auto", "gather"])
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("box", [(24, 24, 24), (7, 9, 10), (1, 1, 37), (13, 1, 5)])
+def test_boxes(box, periodic, kernel):
+    n = 4
+    if periodic and min(box) == 1:
+        n = 2
+    p = Problem(None, None, None, 0.25, max_n=4, box=box, periodic=periodic)
+    rng = np.random.default_rng(17)
+    psi = rng.standard_normal((3, p.np)) + 1j * rng.standard_normal((3, p.np))
+    g = _run(p, psi, n, 2, kernel)
+    o = p.oracle_hpsi(psi, n)
+    check(g, o, p.cond_denominator(psi, n), f"box {box} periodic={periodic}")
+
+
+def test_plane_wave_closed_form_on_gpu():
+    """P5 on the CUDA path itself: periodic 24^3 box, plane wave, closed-form FD symbol."""
+    import math
+
+    n, h, N, m = 4, 0.25, 24, (2, 3, 5)
+    p = Problem(None, None, None, h, max_n=4, box=(N, N, N), periodic=True)
+    p.v_canon[:] = 0.75
+    p.v_mesh[:] = 0.75
+    ijk = p.omesh.ijk().astype(np.float64)
+    q = [2 * math.pi * ma / (N * h) for ma in m]
+    psi = np.exp(1j * sum(q[a] * ijk[:, a] * h for a in range(3)))[None, :]
+    c = [-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560]
+    lam = [(c[0] + 2 * sum(c[k] * math.cos(k * q[a] * h) for k in range(1, n + 1))) / h ** 2 for a in range(3)]
+    expect = (-0.5 * sum(lam) + 0.75) * psi
+    g = p.gpu_hpsi(psi, n, 1, coeffs=np.array(c))
+    assert np.abs(g - expect).max() / np.abs(expect).max() <= 1e-13
+
+
+def test_delta_response_on_gpu():
+    """P8 on the CUDA path: H delta = the star itself (validates every arm of the neighbour structure)."""
+    p = problem(0)
+    n = 4
+    c = oracle.fd_coeffs(n)
+    ijk = p.omesh.ijk()
+    for ctr in ((0, 0, 0), (3, -2, 5), (0, 0, 13), (-9, 4, 2)):
+        ic = int(np.flatnonzero((ijk == np.array(ctr)).all(axis=1))[0])
+        psi = np.zeros((1, p.np))
+        psi[0, ic] = 1.0
+        g = p.gpu_hpsi(psi, n, 1)[0]
+        h = p.cfg.spacing
+        expect = np.zeros(p.np)
+        d = ijk - np.array(ctr)
+        for a in range(3):
+            on_axis = (np.delete(d, a, axis=1) == 0).all(axis=1)
+            for k in range(1, n + 1):
+                expect[on_axis & (np.abs(d[:, a]) == k)] = -0.5 * c[k] / h ** 2
+        expect[ic] = -0.5 * 3 * c[0] / h ** 2 + p.v_canon[ic]
+        assert np.abs(g - expect).max() <= 16 * EPS * np.abs(expect).max(), ctr
+
+
+def test_hermiticity_on_gpu():
+    p = problem(1)
+    phi = synthetic.orbital(101, 0, p.np, True)
+    psi = synthetic.orbital(101, 1, p.np, True)
+    hphi, hpsi = p.gpu_hpsi(np.stack([phi, psi]), 4, 2)
+    assert abs(np.vdot(phi, hpsi) - np.vdot(hphi, psi)) / (np.linalg.norm(phi) * np.linalg.norm(hpsi)) <= 1e-13
+
+
+# ---- pack / unpack: bit-exact against the oracle's layout transform -----------------------------
+@pytest.mark.parametrize("is_complex", [False, True])
+@pytest.mark.parametrize("B", [1, 2, 4, 8, 16, 32, 64])
+def test_pack_unpack_bit_exact(B, is_complex):
+    import torch
+
+    p = problem(0)
+    npts = p.np
+    nst, ld = 11, npts + 3
+    rng = np.random.default_rng(B)
+    st = rng.standard_normal((nst, ld))
+    if is_complex:
+        st = st + 1j * rng.standard_normal((nst, ld))
+    dst = torch.from_numpy(st).cuda()
+    back = torch.full_like(dst, -7.0)
+    tdt = torch.complex128 if is_complex else torch.float64
+    for ist0 in range(0, nst, B):
+        nb = min(B, nst - ist0)
+        blk = torch.full((npts + 1, B), 5.0, dtype=tdt, device="cuda")
+        rs.rs_block_pack(p.mesh, dst, ist0, nb, B, blk)
+        want = oracle.block_pack(st, ist0, nb, B, npts, npts + 1)
+        assert np.array_equal(blk.cpu().numpy(), want)            # zero slot row and padding columns included
+        rs.rs_block_unpack(p.mesh, blk, B, nb, back, ist0)
+    res = back.cpu().numpy()
+    assert np.array_equal(res[:, :npts], st[:, :npts]) and np.all(res[:, npts:] == -7.0)
+
+
+def test_fig4_worked_example_on_gpu():
+    """PAPER.md:107 (Fig. 4): 4 orbitals x 5 coefficients, blocked address = p*4 + j."""
+    import torch
+
+    m = rs.rs_mesh_create_box(5, 1, 1, 1.0, 1, False, rs.RS_ORDER_LEX)
+    st = torch.arange(20, dtype=torch.float64, device="cuda").reshape(4, 5)
+    blk = torch.empty((6, 4), dtype=torch.float64, device="cuda")
+    rs.rs_block_pack(m, st, 0, 4, 4, blk)
+    flat = blk.cpu().numpy().ravel()
+    for j in range(4):
+        for pt in range(5):
+            assert flat[pt * 4 + j] == j * 5 + pt
+    assert np.all(flat[20:] == 0)
+
+
+def test_states_host_entry_point():
+    """Whole path on host buffers (step a7) = per-block device path = oracle."""
+    p = problem(0)
+    psi = synthetic.orbitals(9, 0, 7, p.np, is_complex=True)
+    st = p.to_mesh(psi)
+    out = np.zeros_like(st)
+    rs.rs_hamiltonian_apply_states_host(p.mesh, 4, oracle.fd_coeffs(4), p.v_mesh, st, out, 4)
+    o = p.oracle_hpsi(psi, 4)
+    check(p.to_canon(out), o, p.cond_denominator(psi, 4), "states_host")
+
+
+def test_kernel_choice_is_reported():
+    p = problem(1)
+    name = rs.rs_kernel_name(p.mesh, 4, 16)
+    assert name in ("gather", "brick")
+    assert rs.rs_kernel_table_bytes(p.mesh, 4, 16, kernel=rs.RS_KERNEL_GATHER) == p.np * 24 * 4

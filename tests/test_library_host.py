@@ -1,0 +1,192 @@
+"""Host-side checks of librs.so that need no GPU: the library loads and exports every symbol of
+include/rs.h; the mesh builder (steps a1-a3) agrees with the oracle's own mask as a point SET and
+arm by arm; argument errors are reported as include/rs.h says.  No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import synthetic
+import paper_1306_2953_b200 as rs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "rs.h")).read()
+    body = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(rs_[a-z_0-9]+)\s*\(", body))
+    assert declared == set(rs.EXPORTS), declared ^ set(rs.EXPORTS)
+    lib = C.CDLL(rs.LIBRARY_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert rs.rs_version() >= 100
+
+
+def test_binding_never_imports_oracle():
+    src = open(os.path.join(ROOT, "paper_1306_2953_b200", "__init__.py")).read()
+    src += open(os.path.join(ROOT, "paper_1306_2953_b200", "build.py")).read()
+    assert "oracle" not in src
+    for f in os.listdir(os.path.join(ROOT, "paper_1306_2953_b200", "csrc")):
+        assert "oracle" not in open(os.path.join(ROOT, "paper_1306_2953_b200", "csrc", f)).read().lower(), f
+    osrc = open(os.path.join(ROOT, "oracle", "oracle.c")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert "rs.h" not in osrc and "import paper_1306" not in osrc and "librs" not in osrc
+
+
+def _sets_equal(lib_ijk, omesh):
+    a = set(map(tuple, lib_ijk.tolist()))
+    b = set(map(tuple, omesh.ijk().tolist()))
+    return a == b, (a - b, b - a)
+
+
+@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX])
+@pytest.mark.parametrize("cfg_i", [0, 1])
+def test_mesh_point_set_equals_oracle(cfg_i, ordering):
+    cfg = synthetic.config(cfg_i)
+    m = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, 6, ordering)
+    om = oracle.mesh_from_spheres(cfg.centers, cfg.radius, cfg.spacing)
+    assert m.npoints == om.npoints == cfg.np_expected
+    ijk = m.points()
+    assert len(set(map(tuple, ijk.tolist()))) == m.npoints          # no duplicates
+    ok, diff = _sets_equal(ijk, om)
+    assert ok, diff
+    if ordering == rs.RS_ORDER_LEX:
+        assert np.array_equal(ijk, om.ijk())
+        assert np.array_equal(synthetic.canonical_rank(ijk), np.arange(m.npoints))
+    else:
+        assert m.nbricks > 0
+    # canonical_rank agrees with the oracle's own ranking of the same points
+    assert np.array_equal(synthetic.canonical_rank(ijk), om.canonical_rank_of(ijk))
+
+
+def test_mesh_table1_benzene_count():
+    c, _ = synthetic.benzene_centers()
+    assert rs.rs_mesh_create(c, 5.5, 0.41, 4).npoints == 37295      # PAPER.md:513 prints 37.3k
+
+
+def test_mesh_off_lattice_centres_and_negative_coordinates():
+    rng = np.random.default_rng(3)
+    c = rng.uniform(-3.0, 3.0, (5, 3)) + np.array([-7.3, 2.1, 0.4])
+    m = rs.rs_mesh_create(c, 2.7, 0.33, 4)
+    om = oracle.mesh_from_spheres(c, 2.7, 0.33)
+    ok, diff = _sets_equal(m.points(), om)
+    assert ok, diff
+
+
+def _bruteforce_map(ijk, n, periodic_box=None):
+    """neighbour table from the definition, through a python dict (independent of both builders)."""
+    lut = {tuple(p): i for i, p in enumerate(ijk.tolist())}
+    npts = len(lut)
+    out = np.full((npts, 6 * n), npts, dtype=np.int32)
+    for ip, p in enumerate(ijk.tolist()):
+        for a in range(3):
+            for k in range(1, n + 1):
+                for sgn, d in ((0, k), (1, -k)):
+                    q = list(p)
+                    q[a] += d
+                    if periodic_box is not None:
+                        q[a] %= periodic_box[a]
+                    out[ip, a * 2 * n + 2 * (k - 1) + sgn] = lut.get(tuple(q), npts)
+    return out
+
+
+@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX])
+@pytest.mark.parametrize("n", [1, 4, 6])
+def test_index_map_matches_definition_and_invariants(n, ordering):
+    cfg = synthetic.config(0)
+    m = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, 6, ordering)
+    npts = m.npoints
+    mp = m.index_map(n)
+    assert mp.shape == (npts, 6 * n)
+    assert mp.min() >= 0 and mp.max() <= npts
+    assert np.array_equal(mp, _bruteforce_map(m.points(), n))
+    # P11: map(map(ip,+k),-k) == ip wherever the forward entry is a real point
+    for a in range(3):
+        for k in range(1, n + 1):
+            fwd = mp[:, a * 2 * n + 2 * (k - 1)]
+            real = fwd < npts
+            back = mp[fwd[real], a * 2 * n + 2 * (k - 1) + 1]
+            assert np.array_equal(back, np.flatnonzero(real))
+    # P11: number of zero-slot entries == the oracle's count of star arms leaving the domain
+    om = oracle.mesh_from_spheres(cfg.centers, cfg.radius, cfg.spacing)
+    assert int((mp == npts).sum()) == oracle.count_outside_arms(om, n)
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+def test_box_mesh_and_map(periodic):
+    nx, ny, nz, n = 7, 9, 10, 4
+    m = rs.rs_mesh_create_box(nx, ny, nz, 0.3, n, periodic)
+    assert m.npoints == nx * ny * nz
+    ijk = m.points()
+    assert ijk.min() == 0 and tuple(ijk.max(axis=0)) == (nx - 1, ny - 1, nz - 1)
+    mp = m.index_map(n)
+    assert np.array_equal(mp, _bruteforce_map(ijk, n, (nx, ny, nz) if periodic else None))
+    if periodic:
+        assert mp.max() < m.npoints            # no arm ever leaves a periodic box
+    else:
+        om = oracle.mesh_box(nx, ny, nz, 0.3, False)
+        assert int((mp == m.npoints).sum()) == oracle.count_outside_arms(om, n)
+
+
+def test_block_bytes_and_argument_errors():
+    m = rs.rs_mesh_create(np.zeros((1, 3)), 2.0, 0.5, 4)
+    npts = m.npoints
+    assert rs.rs_block_bytes(m, 16, rs.RS_REAL64) == (npts + 1) * 16 * 8
+    assert rs.rs_block_bytes(m, 8, rs.RS_COMPLEX128) == (npts + 1) * 8 * 16
+    assert rs.rs_block_bytes(m, 3, rs.RS_REAL64) == 0 and rs.rs_block_bytes(m, 128, rs.RS_REAL64) == 0
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_mesh_create(np.zeros((1, 3)), -1.0, 0.5, 4)
+    assert e.value.status == rs.RS_ERR_INVALID_ARG
+    with pytest.raises(rs.RsError):
+        rs.rs_mesh_create(np.zeros((1, 3)), 2.0, 0.5, rs.RS_MAX_FD_ORDER + 1)
+    with pytest.raises(rs.RsError):
+        m.index_map(5)                         # > max_fd_order of this mesh
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_mesh_create(np.array([[100.2, 0.2, 0.2]]), 0.01, 0.5, 4)   # sphere holds no lattice point
+    assert e.value.status == rs.RS_ERR_INVALID_ARG
+
+
+def test_compute_calls_validate_arguments_before_touching_the_device():
+    """Argument errors come back as RS_ERR_INVALID_ARG with or without a GPU (no launch is made)."""
+    m = rs.rs_mesh_create(np.zeros((1, 3)), 2.0, 0.5, 4)
+    npts = m.npoints
+    c = np.array([-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560])
+    v = np.zeros(npts)
+    a = np.zeros((npts + 1) * 4)
+    b = np.zeros((npts + 1) * 4)
+    for bad in (dict(nst=3), dict(nst=128), dict(fd_order=0), dict(fd_order=5), dict(alias=True)):
+        nst = bad.get("nst", 4)
+        n = bad.get("fd_order", 4)
+        cc = c if n == 4 else np.zeros(n + 1)
+        with pytest.raises(rs.RsError) as e:
+            rs.rs_hamiltonian_apply(m, n, cc, v, a, a if bad.get("alias") else b, nst, rs.RS_REAL64, stream=0)
+        assert e.value.status == rs.RS_ERR_INVALID_ARG, bad
+    st = np.zeros((2, npts))
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_block_pack(m, st, 0, 5, 4, a, stream=0)           # nst_in_block > block_size
+    assert e.value.status == rs.RS_ERR_INVALID_ARG
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_block_unpack(m, a, 4, 2, st, 0, stream=0, ld=npts - 1)   # ld < np
+    assert e.value.status == rs.RS_ERR_INVALID_ARG
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    m = rs.rs_mesh_create(np.zeros((1, 3)), 2.0, 0.5, 4)
+    npts = m.npoints
+    c = np.array([-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560])
+    a = np.zeros((npts + 1) * 4)
+    b = np.zeros((npts + 1) * 4)
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_hamiltonian_apply(m, 4, c, np.zeros(npts), a, b, 4, rs.RS_REAL64, stream=0)
+    assert e.value.status == rs.RS_ERR_CUDA
+    assert np.all(b == 0)
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_hamiltonian_apply_states_host(m, 4, c, np.zeros(npts), np.zeros((4, npts)), np.zeros((4, npts)), 4)
+    assert e.value.status == rs.RS_ERR_CUDA
