@@ -176,7 +176,7 @@ def main() -> None:
     ap.add_argument("--block", type=int, default=16)
     ap.add_argument("--fd-order", type=int, default=0)
     ap.add_argument("--nst", type=int, default=0, help="override the orbital count (debugging only; invalidates the number)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "brick"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "sweep"])
     ap.add_argument("--sweep", action="store_true", help="also time apply alone for every block size of the config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -204,7 +204,7 @@ def main() -> None:
     n = args.fd_order or cfg.fd_orders[0]
     B = args.block
     nst = args.nst or cfg.nst
-    kern = {"auto": rs.RS_KERNEL_AUTO, "gather": rs.RS_KERNEL_GATHER, "brick": rs.RS_KERNEL_BRICK}[args.kernel]
+    kern = {"auto": rs.RS_KERNEL_AUTO, "gather": rs.RS_KERNEL_GATHER, "sweep": rs.RS_KERNEL_SWEEP}[args.kernel]
     coeffs = fd_coeffs(n)
     is_c = cfg.is_complex
     rsdt = rs.RS_COMPLEX128 if is_c else rs.RS_REAL64

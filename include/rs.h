@@ -18,8 +18,8 @@
  * Conventions
  *   - "host"/"dev" on every pointer says where the memory lives.  The caller owns every buffer it
  *     passes; the mesh handle owns its own host tables and device tables.
- *   - Mesh order: the library chooses the enumeration of the np in-domain points (brick order, see
- *     DESIGN.md); rs_mesh_get_points() publishes it.  Every per-point array (vloc, states, block
+ *   - Mesh order: the library chooses the enumeration of the np in-domain points (z-rows in
+ *     lexicographic order by default); rs_mesh_get_points() publishes it.  Every per-point array (vloc, states, block
  *     rows) is indexed by that order.
  *   - Block layout: [nrows][ldb] elements, nrows = np + 1, ldb = B.  Row np is the ZERO SLOT: pack
  *     writes zeros there, apply never writes it, and apply REQUIRES it to be zero in psi.  Columns
@@ -59,15 +59,16 @@ typedef enum { RS_REAL64 = 0, RS_COMPLEX128 = 1 } rs_dtype;
 /* Point enumeration (sec. V.A, Fig. 7: "enumerate the grid points based on a
  * sequence of small parallelepipedic grids").  Results do not depend on it beyond rounding order. */
 typedef enum {
-    RS_ORDER_BRICK = 0, /* 4x4x4 bricks, brick after brick (default; enables the brick kernel) */
-    RS_ORDER_LEX = 1    /* lexicographic (i, j, k), k fastest: the paper's "standard order"    */
+    RS_ORDER_BRICK = 0, /* the paper's 4x4x4 bricks, brick after brick (gather kernel only; ablation of Fig. 8) */
+    RS_ORDER_LEX = 1    /* lexicographic (i, j, k), k fastest (default; what the plane-sweep kernel streams)    */
 } rs_ordering;
 
 /* Kernel selection for rs_hamiltonian_apply_v (tests and ablations; results agree to rounding). */
 typedef enum {
     RS_KERNEL_AUTO = 0,   /* best available for this mesh / order / width                         */
     RS_KERNEL_GATHER = 1, /* per-point neighbour table, one gathered load per star arm (any mesh) */
-    RS_KERNEL_BRICK = 2   /* brick-tiled shared-memory kernel (RS_ORDER_BRICK, non-periodic)      */
+    RS_KERNEL_SWEEP = 2   /* plane-sweep kernel: smem-staged planes + register x-window (RS_ORDER_LEX,
+                             non-periodic mesh, fd_order with a compiled variant)                  */
 } rs_kernel;
 
 #define RS_MAX_FD_ORDER 8
@@ -95,7 +96,7 @@ int64_t rs_mesh_nbricks(const rs_mesh *mesh);           /* number of non-empty 4
 rs_status rs_mesh_get_points(const rs_mesh *mesh, int32_t *ijk_host);
 /* map_host [np][6*fd_order] int32: entry (ip, s) is the mesh index of the point at arm s of ip, or np
  * (the zero slot) if that point is outside the mesh.  Arm order: s = axis*2n + 2*(k-1) + (0 for +k,
- * 1 for -k), axis 0 = i, k = 1..n.  This is the table of PAPER.md:131 in its plain form; the brick
+ * 1 for -k), axis 0 = i, k = 1..n.  This is the table of PAPER.md:131 in its plain form; the sweep
  * kernel uses a compact form that expands to exactly this (reading S15).                           */
 rs_status rs_mesh_get_index_map(const rs_mesh *mesh, int fd_order, int32_t *map_host);
 
@@ -139,11 +140,14 @@ rs_status rs_hamiltonian_apply_states_host(const rs_mesh *mesh, int fd_order, co
                                            rs_dtype dtype);
 
 const char *rs_last_error(void);
-/* Static description of the kernel rs_hamiltonian_apply would pick ("gather", "brick", ...).       */
+/* Static description of the kernel rs_hamiltonian_apply would pick ("gather", "sweep[...]").       */
 const char *rs_kernel_name(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, rs_kernel kernel);
 /* Bytes of neighbour structure the chosen kernel reads per call (for the roofline's algorithmic bytes). */
 int64_t rs_kernel_table_bytes(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, rs_kernel kernel);
 int rs_version(void);
+/* Tuning knobs for tests and ablations (not needed for normal use).  "sweep_planes": x-chunk length of a
+ * plane-sweep work item; takes effect for meshes created afterwards.  Unknown name -> RS_ERR_INVALID_ARG. */
+rs_status rs_set_tuning(const char *name, int value);
 
 #ifdef __cplusplus
 }

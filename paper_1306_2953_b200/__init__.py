@@ -24,7 +24,7 @@ from . import build as _build
 RS_OK, RS_ERR_INVALID_ARG, RS_ERR_ALLOC, RS_ERR_CUDA, RS_ERR_UNSUPPORTED = range(5)
 RS_REAL64, RS_COMPLEX128 = 0, 1
 RS_ORDER_BRICK, RS_ORDER_LEX = 0, 1
-RS_KERNEL_AUTO, RS_KERNEL_GATHER, RS_KERNEL_BRICK = 0, 1, 2
+RS_KERNEL_AUTO, RS_KERNEL_GATHER, RS_KERNEL_SWEEP = 0, 1, 2
 RS_MAX_FD_ORDER = 8
 RS_MAX_BLOCK = 64
 
@@ -35,7 +35,7 @@ EXPORTS = (
     "rs_mesh_create", "rs_mesh_create_ordered", "rs_mesh_create_box", "rs_mesh_destroy", "rs_mesh_npoints",
     "rs_mesh_spacing", "rs_mesh_nbricks", "rs_mesh_get_points", "rs_mesh_get_index_map", "rs_block_bytes",
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
-    "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version",
+    "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version", "rs_set_tuning",
 )
 
 
@@ -47,10 +47,11 @@ class RsError(RuntimeError):
 
 def _load() -> C.CDLL:
     so = _build.SO
-    if not os.path.exists(so):
+    if _build.needs_build():
         if shutil.which(os.environ.get("NVCC", "nvcc")) is None:
-            raise ImportError(f"{so} is missing and nvcc is not available to build it; there is no fallback path")
-        _build.build()
+            raise ImportError(f"{so} is missing or stale and nvcc is not available to build it; "
+                              "there is no fallback path")
+        _build.build(force=True, verbose=bool(os.environ.get("RS_BUILD_VERBOSE")))
     L = C.CDLL(so)
     vp, dp, i32p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int32)
     L.rs_mesh_create.argtypes = [dp, C.c_int, C.c_double, C.c_double, C.c_int, C.POINTER(vp)]
@@ -78,6 +79,7 @@ def _load() -> C.CDLL:
     L.rs_kernel_table_bytes.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
     L.rs_kernel_table_bytes.restype = C.c_int64
     L.rs_version.restype = C.c_int
+    L.rs_set_tuning.argtypes = [C.c_char_p, C.c_int]
     return L
 
 
@@ -161,8 +163,12 @@ def rs_version() -> int:
     return int(_lib.rs_version())
 
 
+def rs_set_tuning(name: str, value: int) -> None:
+    _check(_lib.rs_set_tuning(name.encode(), value))
+
+
 def rs_mesh_create(centers, radius: float, spacing: float, max_fd_order: int = 4,
-                   ordering: int = RS_ORDER_BRICK) -> Mesh:
+                   ordering: int = RS_ORDER_LEX) -> Mesh:
     c = np.ascontiguousarray(centers, dtype=np.float64).reshape(-1, 3)
     out = C.c_void_p()
     _check(_lib.rs_mesh_create_ordered(_dptr(c), c.shape[0], radius, spacing, max_fd_order, ordering, C.byref(out)))
@@ -170,7 +176,7 @@ def rs_mesh_create(centers, radius: float, spacing: float, max_fd_order: int = 4
 
 
 def rs_mesh_create_box(nx: int, ny: int, nz: int, spacing: float, max_fd_order: int = 4, periodic: bool = False,
-                       ordering: int = RS_ORDER_BRICK) -> Mesh:
+                       ordering: int = RS_ORDER_LEX) -> Mesh:
     out = C.c_void_p()
     _check(_lib.rs_mesh_create_box(nx, ny, nz, spacing, max_fd_order, int(periodic), ordering, C.byref(out)))
     return Mesh(out.value)

@@ -7,6 +7,7 @@ repository snapshot to the GPU box; it is git-ignored.
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -17,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 SO = os.path.join(HERE, "librs.so")
 
-SOURCES = ["rs_api.cu", "rs_mesh.cu", "rs_kernels.cu", "rs_brick.cu"]
+SOURCES = ["rs_api.cu", "rs_mesh.cu", "rs_kernels.cu", "rs_sweep.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
@@ -27,17 +28,26 @@ NVCC_FLAGS = [
 
 
 def _deps() -> list[str]:
-    d = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    d += [os.path.join(INCLUDE, f) for f in os.listdir(INCLUDE)]
+    d = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".h", ".cuh"))]
+    d += [os.path.join(INCLUDE, f) for f in os.listdir(INCLUDE) if f.endswith(".h")]
     d.append(os.path.abspath(__file__))
     return d
 
 
+def _digest() -> str:
+    h = hashlib.sha256()
+    for p in sorted(_deps()):
+        h.update(os.path.basename(p).encode())
+        h.update(open(p, "rb").read())
+    return h.hexdigest()
+
+
 def needs_build() -> bool:
-    if not os.path.exists(SO):
+    """True when librs.so is missing or was built from other sources (content hash, not mtime:
+    the snapshot that carries the tree to the GPU box does not promise to keep mtimes)."""
+    if not os.path.exists(SO) or not os.path.exists(SO + ".sha256"):
         return True
-    t = os.path.getmtime(SO)
-    return any(os.path.getmtime(p) > t for p in _deps())
+    return open(SO + ".sha256").read().strip() != _digest()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -53,6 +63,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
     if verbose:
         sys.stderr.write(r.stderr)
+    with open(SO + ".sha256", "w") as f:
+        f.write(_digest())
     return SO
 
 

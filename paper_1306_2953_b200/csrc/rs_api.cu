@@ -41,7 +41,7 @@ static rs_status check_apply(const rs_mesh *m, int n, const double *coeffs, cons
 
 static rs_kernel resolve_kernel(const rs_mesh *m, int n, int ncol, rs_kernel k)
 {
-    if (k == RS_KERNEL_AUTO) return rs_brick_supported(m, n, ncol) ? RS_KERNEL_BRICK : RS_KERNEL_GATHER;
+    if (k == RS_KERNEL_AUTO) return rs_sweep_supported(m, n, ncol) ? RS_KERNEL_SWEEP : RS_KERNEL_GATHER;
     return k;
 }
 
@@ -57,9 +57,9 @@ extern "C" rs_status rs_hamiltonian_apply_v(const rs_mesh *m, int n, const doubl
     for (int k = 0; k <= n; ++k) w.w[k] = -0.5 * coeffs[k] / (m->h * m->h);
     const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);  // complex = 2 independent real columns
     const rs_kernel k = resolve_kernel(m, n, ncol, kernel);
-    if (k == RS_KERNEL_BRICK) {
-        if (!rs_brick_supported(m, n, ncol)) return rs_fail(RS_ERR_UNSUPPORTED, "brick kernel cannot serve this call");
-        return rs_launch_brick(m, n, w, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
+    if (k == RS_KERNEL_SWEEP) {
+        if (!rs_sweep_supported(m, n, ncol)) return rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep kernel cannot serve this call");
+        return rs_launch_sweep(m, n, w, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
     }
     if (k != RS_KERNEL_GATHER) return rs_fail(RS_ERR_INVALID_ARG, "unknown kernel id");
     const int32_t *d_map = nullptr;
@@ -78,14 +78,14 @@ extern "C" const char *rs_kernel_name(const rs_mesh *m, int n, int nst, rs_dtype
 {
     if (!m) return "none";
     const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
-    return resolve_kernel(m, n, ncol, kernel) == RS_KERNEL_BRICK ? "brick" : "gather";
+    return resolve_kernel(m, n, ncol, kernel) == RS_KERNEL_SWEEP ? rs_sweep_variant_name(m, n, ncol) : "gather";
 }
 
 extern "C" int64_t rs_kernel_table_bytes(const rs_mesh *m, int n, int nst, rs_dtype dtype, rs_kernel kernel)
 {
     if (!m) return 0;
     const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
-    if (resolve_kernel(m, n, ncol, kernel) == RS_KERNEL_BRICK) return rs_brick_table_bytes(m);
+    if (resolve_kernel(m, n, ncol, kernel) == RS_KERNEL_SWEEP) return rs_sweep_table_bytes(m, n, ncol);
     return m->np * 6 * (int64_t)n * 4;
 }
 
@@ -141,4 +141,14 @@ extern "C" rs_status rs_hamiltonian_apply_states_host(const rs_mesh *m, int n, c
     cleanup();
 #undef TRY_OR_CLEAN
     return RS_OK;
+}
+
+void rs_sweep_set_max_planes(int v);
+extern "C" rs_status rs_set_tuning(const char *name, int value)
+{
+    if (name && std::strcmp(name, "sweep_planes") == 0) {
+        rs_sweep_set_max_planes(value);
+        return RS_OK;
+    }
+    return rs_fail(RS_ERR_INVALID_ARG, "rs_set_tuning: unknown knob");
 }

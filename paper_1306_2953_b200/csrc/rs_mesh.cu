@@ -1,6 +1,7 @@
 // Host mesh builder: steps a1-a3 of SURVEY.md section 8(a).
 //   a1  enumerate the lattice points in the union of closed balls   (PAPER.md:53 sec. II; :354 sec. XII)
-//   a2  choose the point enumeration: 4x4x4 bricks                   (sec. V.A, Fig. 7)
+//   a2  choose the point enumeration: lexicographic z-rows (default; what the plane-sweep kernel
+//       streams) or the paper's 4x4x4 bricks                         (sec. V.A, Fig. 7)
 //   a3  neighbour table; outside points map to the zero slot np      (sec. V.A)
 // Everything here runs once per geometry on the host; the tables are uploaded once.
 #include <algorithm>
@@ -22,10 +23,7 @@ extern "C" int rs_version(void) { return 100; }
 
 static inline int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
-static inline size_t dense_index(const rs_mesh *m, int ix, int iy, int iz)
-{
-    return ((size_t)ix * m->dims[1] + iy) * m->dims[2] + iz;
-}
+static inline size_t dense_index(const rs_mesh *m, int ix, int iy, int iz) { return rs_dense_index(m, ix, iy, iz); }
 
 // Order the in-domain cells of `in` (dense [dims]) and fill ijk / dense2point / brick tables.
 static void enumerate_points(rs_mesh *m, const std::vector<uint8_t> &in)
@@ -48,35 +46,20 @@ static void enumerate_points(rs_mesh *m, const std::vector<uint8_t> &in)
         m->np = count;
         return;
     }
-    for (int a = 0; a < 3; ++a) m->nb[a] = m->dims[a] / RS_BRICK;
-    m->cell2brick.assign((size_t)m->nb[0] * m->nb[1] * m->nb[2], -1);
-    m->boff.clear();
-    m->bmask.clear();
-    m->bcoord.clear();
-    for (int bx = 0; bx < m->nb[0]; ++bx)
-        for (int by = 0; by < m->nb[1]; ++by)
-            for (int bz = 0; bz < m->nb[2]; ++bz) {
-                uint64_t mask = 0;
-                const int32_t first = (int32_t)count;
+    // paper's enumeration: brick after brick, points inside a brick in (x, y, z) order
+    const int nb[3] = {m->dims[0] / RS_BRICK, m->dims[1] / RS_BRICK, m->dims[2] / RS_BRICK};
+    m->nbricks = 0;
+    for (int bx = 0; bx < nb[0]; ++bx)
+        for (int by = 0; by < nb[1]; ++by)
+            for (int bz = 0; bz < nb[2]; ++bz) {
+                const int64_t first = count;
                 for (int p = 0; p < RS_BRICK_PTS; ++p) {
                     const int ix = bx * RS_BRICK + (p >> 4), iy = by * RS_BRICK + ((p >> 2) & 3),
                               iz = bz * RS_BRICK + (p & 3);
-                    if (in[dense_index(m, ix, iy, iz)]) {
-                        mask |= (uint64_t)1 << p;
-                        push(ix, iy, iz);
-                    }
+                    if (in[dense_index(m, ix, iy, iz)]) push(ix, iy, iz);
                 }
-                if (mask) {
-                    m->cell2brick[((size_t)bx * m->nb[1] + by) * m->nb[2] + bz] = (int32_t)m->bmask.size();
-                    m->boff.push_back(first);
-                    m->bmask.push_back(mask);
-                    m->bcoord.push_back(bx);
-                    m->bcoord.push_back(by);
-                    m->bcoord.push_back(bz);
-                }
+                if (count > first) ++m->nbricks;
             }
-    m->boff.push_back((int32_t)count);
-    m->nbricks = (int64_t)m->bmask.size();
     m->np = count;
 }
 
@@ -91,19 +74,6 @@ static rs_status upload(rs_mesh *m)
     RS_CUDA_TRY(cudaGetDevice(&m->device));
     RS_CUDA_TRY(cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, m->device));
     m->have_device = true;
-    if (m->ordering == RS_ORDER_BRICK && m->nbricks > 0) {
-        RS_CUDA_TRY(cudaMalloc(&m->d_cell2brick, m->cell2brick.size() * sizeof(int32_t)));
-        RS_CUDA_TRY(cudaMalloc(&m->d_boff, m->boff.size() * sizeof(int32_t)));
-        RS_CUDA_TRY(cudaMalloc(&m->d_bmask, m->bmask.size() * sizeof(uint64_t)));
-        RS_CUDA_TRY(cudaMalloc(&m->d_bcoord, m->bcoord.size() * sizeof(int32_t)));
-        RS_CUDA_TRY(cudaMemcpy(m->d_cell2brick, m->cell2brick.data(), m->cell2brick.size() * sizeof(int32_t),
-                               cudaMemcpyHostToDevice));
-        RS_CUDA_TRY(cudaMemcpy(m->d_boff, m->boff.data(), m->boff.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-        RS_CUDA_TRY(cudaMemcpy(m->d_bmask, m->bmask.data(), m->bmask.size() * sizeof(uint64_t), cudaMemcpyHostToDevice));
-        RS_CUDA_TRY(cudaMemcpy(m->d_bcoord, m->bcoord.data(), m->bcoord.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-        rs_status st = rs_brick_prepare(m);
-        if (st != RS_OK) return st;
-    }
     return RS_OK;
 }
 
@@ -191,7 +161,7 @@ extern "C" rs_status rs_mesh_create_ordered(const double *centers, int nc, doubl
 extern "C" rs_status rs_mesh_create(const double *centers, int nc, double radius, double spacing, int max_fd_order,
                                     rs_mesh **out)
 {
-    return rs_mesh_create_ordered(centers, nc, radius, spacing, max_fd_order, RS_ORDER_BRICK, out);
+    return rs_mesh_create_ordered(centers, nc, radius, spacing, max_fd_order, RS_ORDER_LEX, out);
 }
 
 extern "C" rs_status rs_mesh_create_box(int nx, int ny, int nz, double spacing, int max_fd_order, int periodic,
@@ -226,12 +196,7 @@ extern "C" rs_status rs_mesh_destroy(rs_mesh *m)
     if (m->have_device) {
         for (int n = 0; n <= RS_MAX_FD_ORDER; ++n)
             if (m->d_map[n]) cudaFree(m->d_map[n]);
-        if (m->d_cell2brick) cudaFree(m->d_cell2brick);
-        if (m->d_boff) cudaFree(m->d_boff);
-        if (m->d_bmask) cudaFree(m->d_bmask);
-        if (m->d_bcoord) cudaFree(m->d_bcoord);
-        if (m->d_tiles) cudaFree(m->d_tiles);
-        if (m->d_counter) cudaFree(m->d_counter);
+        rs_sweep_free(m);
     }
     delete m;
     return RS_OK;

@@ -19,7 +19,7 @@ EPS = np.finfo(np.float64).eps
 
 
 class Problem:
-    def __init__(self, centers, charges, radius, spacing, max_n=6, ordering=rs.RS_ORDER_BRICK, box=None,
+    def __init__(self, centers, charges, radius, spacing, max_n=6, ordering=rs.RS_ORDER_LEX, box=None,
                  periodic=False):
         if box is None:
             self.mesh = rs.rs_mesh_create(centers, radius, spacing, max_n, ordering)

@@ -11,11 +11,11 @@ from harness import EPS, Problem, check
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = {"auto": rs.RS_KERNEL_AUTO, "gather": rs.RS_KERNEL_GATHER, "brick": rs.RS_KERNEL_BRICK}
+KERNELS = {"auto": rs.RS_KERNEL_AUTO, "gather": rs.RS_KERNEL_GATHER, "sweep": rs.RS_KERNEL_SWEEP}
 _cache = {}
 
 
-def problem(i, ordering=rs.RS_ORDER_BRICK):
+def problem(i, ordering=rs.RS_ORDER_LEX):
     key = (i, ordering)
     if key not in _cache:
         _cache[key] = Problem.from_config(i, ordering=ordering)
@@ -32,7 +32,7 @@ def _run(p, psi, n, B, kernel):
 
 
 # ---- config 0: tiny atom, nst=4, B=4 (BASELINE.json configs[0]) ---------------------------------
-@pytest.mark.parametrize("kernel", ["auto", "gather", "brick"])
+@pytest.mark.parametrize("kernel", ["auto", "gather", "sweep"])
 @pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX])
 def test_config0(kernel, ordering):
     p = problem(0, ordering)
@@ -207,5 +207,5 @@ def test_states_host_entry_point():
 def test_kernel_choice_is_reported():
     p = problem(1)
     name = rs.rs_kernel_name(p.mesh, 4, 16)
-    assert name in ("gather", "brick")
+    assert name in ("gather", "sweep")
     assert rs.rs_kernel_table_bytes(p.mesh, 4, 16, kernel=rs.RS_KERNEL_GATHER) == p.np * 24 * 4
