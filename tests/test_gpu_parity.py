@@ -207,5 +207,5 @@ def test_states_host_entry_point():
 def test_kernel_choice_is_reported():
     p = problem(1)
     name = rs.rs_kernel_name(p.mesh, 4, 16)
-    assert name in ("gather", "sweep")
+    assert name == "gather" or name.startswith("sweep[")
     assert rs.rs_kernel_table_bytes(p.mesh, 4, 16, kernel=rs.RS_KERNEL_GATHER) == p.np * 24 * 4
