@@ -41,7 +41,7 @@ static rs_status check_apply(const rs_mesh *m, int n, const double *coeffs, cons
 
 static rs_kernel resolve_kernel(const rs_mesh *m, int n, int ncol, rs_kernel k)
 {
-    if (k == RS_KERNEL_AUTO) return rs_sweep_supported(m, n, ncol) ? RS_KERNEL_SWEEP : RS_KERNEL_GATHER;
+    if (k == RS_KERNEL_AUTO) return rs_sweep_usable(m, n, ncol) ? RS_KERNEL_SWEEP : RS_KERNEL_GATHER;
     return k;
 }
 

@@ -14,33 +14,31 @@ constexpr int RS_BRICK = 4;                                   // brick edge (poi
 constexpr int RS_BRICK_PTS = RS_BRICK * RS_BRICK * RS_BRICK;  // 64 points
 
 // ---- plane-sweep kernel tables (rs_sweep.cu) -------------------------------------------------------
-// One record per (tile, lattice plane x, tile row r): the compact form of the neighbour table
-// ("a compact form of it is used"; reading S15).  The tile covers lattice rows
-// y = y0 - n + r, r in [0, TY + 2n), and the z window [z0 - n, z0 + TZ + n).  bit zp of `mask` says
-// whether lattice point (x, y0 - n + r, z0 - n + zp) is in the mesh; `off` is the mesh index of the
-// first such point (in-domain points of a z-row are consecutive in RS_ORDER_LEX).  Halo rows carry
-// only the bits of the tile's own z range (the star has no corners).
-struct rs_rowinfo {
-    int32_t off;
-    int32_t pad;
-    uint64_t mask;
+// The compact form of the neighbour table ("a compact form of it is used"; reading S15):
+// one record per (work item, lattice plane).  A work item is a 16 x 16 tile of the (y, z) plane and a
+// range [xa, xb) of x planes; its steps cover planes xa-4 .. xb+3 (the first and last 4 only feed the
+// x arms).  A record holds
+//   runs[RS_SWEEP_MAXRUN]  {first mesh index, destination slot | npoints << 16}: one bulk copy per run of
+//                          consecutive in-domain points of a z-row (consecutive in memory in RS_ORDER_LEX);
+//   fill[16]               2 bits per thread: zero-fill its two plane slots (lattice point outside the mesh);
+//   cidx[256]              mesh index of the tile's own points (-1: outside the mesh / not an output plane);
+//   hdr                    2 bits per warp: 0 no mesh point in the warp's 4 x 8 region, 1 centre-only, 2 full.
+#define RS_SWEEP_MAXRUN 64
+struct rs_sweep_host {
+    std::vector<int2> items;      // {first record, number of steps}
+    std::vector<uint2> runs;
+    std::vector<uint32_t> fill;
+    std::vector<int32_t> cidx;
+    std::vector<uint32_t> hdr;
 };
-static_assert(sizeof(rs_rowinfo) == 16, "rowinfo is read as one 16-byte vector");
-
-// One work item: output planes [xa, xb) of tile (y0, z0); `tab` = index of the record of plane
-// (xa - n), row 0, in the rowinfo array; records of successive planes follow each other.
-struct rs_sweep_item {
-    int32_t y0, z0, xa, xb;
-    int64_t tab;
-};
-
 struct rs_sweep_tables {
-    int n = 0, ty = 0, tz = 0;
-    int64_t nitems = 0;
-    int64_t nrecords = 0;
-    rs_sweep_item *d_items = nullptr;
-    rs_rowinfo *d_rows = nullptr;
-    int64_t active_lanes = 0;   // sum over items of (planes * TY * TZ): dense work incl. masked lanes
+    bool ok = false;              // false: some plane needs more than RS_SWEEP_MAXRUN runs (use the gather kernel)
+    int64_t nitems = 0, nrec = 0, bytes = 0;
+    int2 *d_items = nullptr;
+    uint2 *d_runs = nullptr;
+    uint32_t *d_fill = nullptr;
+    int32_t *d_cidx = nullptr;
+    uint32_t *d_hdr = nullptr;
 };
 
 struct rs_mesh {
@@ -63,7 +61,7 @@ struct rs_mesh {
     int device = -1;
     int sm_count = 0;
     int32_t *d_map[RS_MAX_FD_ORDER + 1] = {nullptr};                 // [np][6n], built lazily per order
-    std::map<std::tuple<int, int, int>, rs_sweep_tables> sweep;      // (n, TY, TZ) -> tables, built lazily
+    std::map<int, rs_sweep_tables> sweep;                            // fd_order -> tables, built lazily
 };
 
 void rs_set_error(const std::string &msg);
@@ -96,12 +94,12 @@ rs_status rs_launch_gather(const rs_mesh *m, int n, const rs_weights &w, const i
                            const double *psi, double *hpsi, int ncol, cudaStream_t st);
 
 // rs_sweep.cu
-bool rs_sweep_supported(const rs_mesh *m, int n, int ncol);
+bool rs_sweep_supported(const rs_mesh *m, int n, int ncol);   // static conditions (ordering, order, width)
+bool rs_sweep_usable(const rs_mesh *m, int n, int ncol);      // supported, device present and tables built
 rs_status rs_launch_sweep(const rs_mesh *m, int n, const rs_weights &w, const double *vloc, const double *psi,
                           double *hpsi, int ncol, cudaStream_t st);
 int64_t rs_sweep_table_bytes(const rs_mesh *m, int n, int ncol);
 const char *rs_sweep_variant_name(const rs_mesh *m, int n, int ncol);
 void rs_sweep_free(rs_mesh *m);
-// host-only construction of the tables (also used by rs_mesh_get_index_map's self-check in tests)
-void rs_sweep_build_host(const rs_mesh *m, int n, int ty, int tz, int max_planes, std::vector<rs_sweep_item> &items,
-                         std::vector<rs_rowinfo> &rows, int64_t *active_lanes);
+// host-only construction of the records; false if a plane needs more than RS_SWEEP_MAXRUN runs
+bool rs_sweep_build_host(const rs_mesh *m, int n, int max_planes, rs_sweep_host &out);

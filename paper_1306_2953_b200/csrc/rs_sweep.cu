@@ -1,481 +1,587 @@
 // Plane-sweep kernel: the fused stencil + local potential (step a5; eq. 2 :41)
-// as a 2.5-D streaming kernel for sm_100a.
+// as a 2.5-D streaming kernel written for sm_100a (TMA bulk copies, mbarriers, tensor memory).
 //
 // What differs from the paper's kernel (one thread per (point, orbital), every star arm
-// a separate load through a neighbour table) and why:
-//   * A CTA owns a (TY x TZ)-point tile of the lattice's (y, z) plane and C of the block's columns and
-//     marches along x.  Plane p of the tile (plus its y/z halos, no corners) is staged in shared
-//     memory once (cp.async, zero-filled where the lattice point is outside the mesh = reading S3);
-//     the x arm never touches memory again: every thread keeps, per output it owns, the last n centre
-//     values and n partial sums in registers (2n-deep register window).
-//   * A thread owns a Q x P patch of (y, z) points and VEC adjacent columns, so the y/z arm operands
-//     it reads from shared memory are shared between its outputs: QP + 2n(Q + P) reads for QP outputs
-//     instead of (4n + 1) QP.  On B200 the shared-memory pipe (128 B/clk/SM), not HBM, bounds a kernel
-//     that reads all 6n + 1 operands per output.
-//   * The neighbour table is the compact per-(tile, plane, row) record {first index, occupancy mask}
-//     of rs_internal.h: ~1 byte per point instead of 24n.
-// Requires RS_ORDER_LEX (in-domain points of a z-row consecutive in memory) and a non-periodic mesh;
-// anything else is served by the gather kernel.
+// a separate load through a neighbour table) and why -- see DESIGN.md "Kernels":
+//   * A CTA owns a 16 x 16 tile of the lattice's (y, z) plane and 16 block columns, and marches along
+//     x.  Plane p of the tile plus its y/z halos (no corners) is staged in shared memory ONCE by
+//     bulk async copies (cp.async.bulk, one per run of in-domain points of a z-row: such a run is
+//     one contiguous span of the blocked array because the orbital index is fastest);
+//     completion is tracked by an mbarrier per stage.  Lattice points outside the mesh are zero-filled
+//     in shared memory (reading S3), so the compute code has no predicates.
+//   * A thread owns a 4 x 4 patch of (y, z) points of ONE column (the 16 lanes of a half-warp are the
+//     16 columns of a point: every shared-memory read is a conflict-free 128-byte row).  The y/z arm
+//     operands are shared inside the patch: 5 shared-memory reads per output instead of 17.
+//   * The x arm never touches shared memory: the forward half is accumulated into the 4 pending
+//     outputs of each (y, z) column held in registers; the backward half needs the centre values of
+//     the previous 4 planes, which are parked in TENSOR MEMORY (tcgen05.st / tcgen05.ld, 32x32b shape:
+//     every thread owns one TMEM lane, i.e. a private 2 KB scratch with ~2.6x the bandwidth of shared
+//     memory, measured).  No tensor-core arithmetic is involved: the path is not a contraction.
+//   * The neighbour table is replaced by per-(tile, plane) records built once on the host: the list of
+//     copy runs, zero-fill bits, the mesh index of each of the tile's 256 points (for V and for the
+//     store) and a 2-bit mode per warp (empty / centre-only / full) that lets a warp skip the planes
+//     in which its 4 x 8 region holds no mesh point.  The records expand to exactly the plain table of
+//     rs_mesh_get_index_map (reading S15).
+// Requires RS_ORDER_LEX (in-domain points of a z-row consecutive in memory), a non-periodic mesh,
+// fd_order 4 and a block of 16 real columns (B = 16 real or B = 8 complex); anything else is served by
+// the gather kernel.
 #include <algorithm>
 
 #include "rs_internal.h"
 
+namespace {
+
+constexpr int SW_N = 4;                  // half-width of the star
+constexpr int SW_T = 16;                 // tile edge (points) in y and z
+constexpr int SW_W = SW_T + 2 * SW_N;    // 24: rows / z-slots of a staged plane
+constexpr int SW_C = 16;                 // columns per CTA
+constexpr int SW_SLOT_BYTES = SW_C * 8;  // 128
+constexpr int SW_STAGE_BYTES = SW_W * SW_W * SW_SLOT_BYTES;  // 73,728: uniform [24][24] slots, corners hold V and idx
+constexpr int SW_STAGES = 3;
+constexpr int SW_THREADS = 256;
+constexpr int SW_MAXRUN = RS_SWEEP_MAXRUN;
+constexpr int SW_TMEM_COLS = 512;        // allocated; used: 2 x (4 x 32 [centre ring] + 4 x 16 [index ring])
+constexpr size_t SW_SMEM = (size_t)SW_STAGES * SW_STAGE_BYTES;
+
 // ---------------------------------------------------------------------------------------------
-// host: tiles, work items, row records
+// PTX wrappers
 // ---------------------------------------------------------------------------------------------
-void rs_sweep_build_host(const rs_mesh *m, int n, int ty, int tz, int max_planes, std::vector<rs_sweep_item> &items,
-                         std::vector<rs_rowinfo> &rows, int64_t *active_lanes)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.expect_tx.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+// one contiguous span global -> shared, completion counted in bytes on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const void *src, uint32_t src_bytes)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_arrive_noinc(uint32_t bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+}
+
+// ---- tensor memory: every thread reads / writes consecutive 32-bit columns of its own lane -------
+#define R4(a, o) "r"(a[o]), "r"(a[o + 1]), "r"(a[o + 2]), "r"(a[o + 3])
+#define W4(a, o) "=r"(a[o]), "=r"(a[o + 1]), "=r"(a[o + 2]), "=r"(a[o + 3])
+#define P4(a, o) "+r"(a[o]), "+r"(a[o + 1]), "+r"(a[o + 2]), "+r"(a[o + 3])
+
+__device__ __forceinline__ void tm_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+        : W4(r, 0), W4(r, 4), W4(r, 8), W4(r, 12)
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tm_ld32(uint32_t taddr, uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,"
+        "%30,%31}, [%32];\n"
+        : W4(r, 0), W4(r, 4), W4(r, 8), W4(r, 12), W4(r, 16), W4(r, 20), W4(r, 24), W4(r, 28)
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tm_st16(uint32_t taddr, const uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};\n" ::"r"(taddr),
+        R4(r, 0), R4(r, 4), R4(r, 8), R4(r, 12)
+        : "memory");
+}
+__device__ __forceinline__ void tm_st32(uint32_t taddr, const uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,"
+        "%31,%32};\n" ::"r"(taddr),
+        R4(r, 0), R4(r, 4), R4(r, 8), R4(r, 12), R4(r, 16), R4(r, 20), R4(r, 24), R4(r, 28)
+        : "memory");
+}
+// The loaded registers are passed through the wait so that no use of them can be scheduled above it.
+__device__ __forceinline__ void tm_wait_ld16(uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" : P4(r, 0), P4(r, 4), P4(r, 8), P4(r, 12)::"memory");
+}
+__device__ __forceinline__ void tm_wait_ld32(uint32_t (&r)[32])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n"
+                 : P4(r, 0), P4(r, 4), P4(r, 8), P4(r, 12), P4(r, 16), P4(r, 20), P4(r, 24), P4(r, 28)::"memory");
+}
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
+#undef R4
+#undef W4
+#undef P4
+
+// ---------------------------------------------------------------------------------------------
+// the kernel
+// ---------------------------------------------------------------------------------------------
+struct sweep_args {
+    const int2 *items;       // {first record, number of steps}
+    const uint2 *runs;       // [nrec][SW_MAXRUN]  {first mesh index, dst slot | npoints << 16}
+    const uint32_t *fill;    // [nrec][16]         2 zero-fill bits per thread
+    const int32_t *cidx;     // [nrec][256]        mesh index of the tile's points (-1: none / not an output plane)
+    const uint32_t *hdr;     // [nrec]             2-bit mode per warp
+    const double *vloc;
+    const double *psi;
+    double *hpsi;
+};
+
+enum { MODE_EMPTY = 0, MODE_CENTRE = 1, MODE_FULL = 2 };
+
+__global__ void __launch_bounds__(SW_THREADS, 1)
+sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_weights w)
+{
+    constexpr int N = SW_N;
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ uint64_t full_bar[SW_STAGES];
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int c = tid & 15, patch = tid >> 4, py = patch >> 2, pz = patch & 3;
+    const int2 item = a.items[blockIdx.x];
+    const size_t rec0 = (size_t)item.x;
+    const int nsteps = item.y;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < SW_STAGES; ++s) mbar_init(smem_u32(&full_bar[s]), SW_THREADS);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_base_s)),
+                     "n"(SW_TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    // this thread's TMEM lane (its warp's quarter) and the column range of its warp
+    const uint32_t tbase = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(warp >> 2) * 192u;
+    const uint32_t t_in = tbase;          // 4 slots x 32 columns: centre values of the last 4 planes (16 doubles each)
+    const uint32_t t_ix = tbase + 128u;   // 4 slots x 16 columns: mesh indices of the last 4 planes' outputs
+
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar0 = smem_u32(&full_bar[0]);
+
+    // ---- loader constants: two plane slots to zero-fill, one tile point for V and the index ----------
+    uint32_t fill_off1, fill_off2;
+    {
+        const int e1 = tid, e2 = tid + 256;
+        fill_off1 = (uint32_t)(((N + e1 / SW_W) * SW_W + e1 % SW_W) * SW_SLOT_BYTES);
+        if (e2 < SW_T * SW_W)
+            fill_off2 = (uint32_t)(((N + e2 / SW_W) * SW_W + e2 % SW_W) * SW_SLOT_BYTES);
+        else {
+            const int q = e2 - SW_T * SW_W, hr = q / SW_T;
+            fill_off2 = (uint32_t)((((hr < N ? hr : hr + SW_T)) * SW_W + N + q % SW_T) * SW_SLOT_BYTES);
+        }
+    }
+    const int ty = tid >> 4, tz = tid & 15;
+    // corner A (rows 0..3, slots 0..3) holds V[16][16]; corner B (rows 0..3, slots 20..23) holds idx[16][16]
+    const uint32_t v_off = (uint32_t)(((ty >> 2) * SW_W) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 8);
+    const uint32_t i_off = (uint32_t)(((ty >> 2) * SW_W + SW_W - N) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 4);
+    // ---- compute constants -------------------------------------------------------------------------
+    const uint32_t b0 = (uint32_t)(((N + 4 * py) * SW_W + 4 * pz) * SW_SLOT_BYTES + c * 8);   // patch row 0, window slot 0
+    const uint32_t vrow = (uint32_t)((py * SW_W) * SW_SLOT_BYTES + (4 * pz) * 8);
+    const uint32_t irow = (uint32_t)((py * SW_W + SW_W - N) * SW_SLOT_BYTES + (4 * pz) * 4);
+
+    // ---- producer: stage plane tl (records prefetched one step ahead in registers) ----------------------
+    int32_t p_cidx;
+    uint32_t p_fill;
+    uint2 p_run0 = make_uint2(0, 0), p_run1 = make_uint2(0, 0);
+    auto prefetch_rec = [&](int tl) {
+        const size_t rec = rec0 + tl;
+        p_cidx = __ldg(a.cidx + rec * 256 + tid);
+        p_fill = __ldg(a.fill + rec * 16 + (tid >> 4));
+        if (warp == 0) {
+            p_run0 = __ldg(a.runs + rec * SW_MAXRUN + lane);
+            p_run1 = __ldg(a.runs + rec * SW_MAXRUN + 32 + lane);
+        }
+    };
+    auto produce = [&](int tl, int stage_l) {
+        const uint32_t sb = sbase + (uint32_t)stage_l * SW_STAGE_BYTES;
+        const uint32_t bar = bar0 + 8u * stage_l;
+        if (warp == 0) {
+            const uint32_t n0 = p_run0.y >> 16, n1 = p_run1.y >> 16;
+            fence_proxy_async();
+            if (n0 + n1) mbar_expect_tx(bar, (n0 + n1) * SW_SLOT_BYTES);
+            if (n0)
+                bulk_g2s(sb + (p_run0.y & 0xffffu) * SW_SLOT_BYTES, a.psi + (size_t)p_run0.x * SW_C, n0 * SW_SLOT_BYTES, bar);
+            if (n1)
+                bulk_g2s(sb + (p_run1.y & 0xffffu) * SW_SLOT_BYTES, a.psi + (size_t)p_run1.x * SW_C, n1 * SW_SLOT_BYTES, bar);
+        }
+        const uint32_t fb = p_fill >> (2 * (tid & 15));
+        if (fb & 1u) {
+            float4 *d = reinterpret_cast<float4 *>(smem + (size_t)stage_l * SW_STAGE_BYTES + fill_off1);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) d[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        if (fb & 2u) {
+            float4 *d = reinterpret_cast<float4 *>(smem + (size_t)stage_l * SW_STAGE_BYTES + fill_off2);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) d[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        *reinterpret_cast<int32_t *>(smem + (size_t)stage_l * SW_STAGE_BYTES + i_off) = p_cidx;
+        cp_async8_zfill(sb + v_off, a.vloc + (p_cidx >= 0 ? p_cidx : 0), p_cidx >= 0 ? 8u : 0u);
+        cp_async_arrive_noinc(bar);
+        if (tl + 1 < nsteps) prefetch_rec(tl + 1);
+    };
+
+    prefetch_rec(0);
+#pragma unroll
+    for (int s = 0; s < SW_STAGES - 1; ++s)
+        if (s < nsteps) produce(s, s);
+
+    double acc[N][4][4];   // pending outputs: acc[t mod 4] belongs to plane t
+#pragma unroll
+    for (int k = 0; k < N; ++k)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc[k][j][i] = 0.0;
+
+    uint32_t hdr_cur = __ldg(a.hdr + rec0);
+    int stage = 0;
+    uint32_t parity = 0;
+    const double w0x3 = 3.0 * w.w[0];
+    double *const hp = a.hpsi + c;
+
+    for (int t0 = 0; t0 < nsteps; t0 += N) {
+#pragma unroll
+        for (int PH = 0; PH < N; ++PH) {
+            const int t = t0 + PH;
+            if (t >= nsteps) break;
+            mbar_wait(bar0 + 8u * stage, parity);
+            __syncthreads();
+            if (t + SW_STAGES - 1 < nsteps) produce(t + SW_STAGES - 1, stage == 0 ? SW_STAGES - 1 : stage - 1);
+            const uint32_t hdr_next = (t + 1 < nsteps) ? __ldg(a.hdr + rec0 + t + 1) : 0u;
+            const int mode = (int)((hdr_cur >> (2 * warp)) & 3u);
+            const unsigned char *sp = smem + (size_t)stage * SW_STAGE_BYTES;
+            const double *pb = reinterpret_cast<const double *>(sp + b0);
+
+            // mesh indices of the outputs completed by this step (plane t - 4), then park this plane's
+            uint32_t io[16];
+            tm_ld16(t_ix + PH * 16, io);
+            uint32_t in_[16];
+            if (mode == MODE_FULL) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int4 q = *reinterpret_cast<const int4 *>(sp + irow + j * 64);
+                    in_[4 * j] = (uint32_t)q.x, in_[4 * j + 1] = (uint32_t)q.y, in_[4 * j + 2] = (uint32_t)q.z,
+                            in_[4 * j + 3] = (uint32_t)q.w;
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < 16; ++q) in_[q] = 0xffffffffu;
+            }
+            tm_wait_ld16(io);
+            tm_st16(t_ix + PH * 16, in_);
+
+            uint32_t cw[32];   // this plane's centre values (16 doubles) as TMEM words
+            if (mode != MODE_EMPTY) {
+                double ctr[4][4];
+                if (mode == MODE_FULL) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        double v[4 + 2 * N];
+#pragma unroll
+                        for (int tt = 0; tt < 4 + 2 * N; ++tt) v[tt] = pb[(j * SW_W + tt) * SW_C];
+                        const double2 va = *reinterpret_cast<const double2 *>(sp + vrow + j * 128);
+                        const double2 vb = *reinterpret_cast<const double2 *>(sp + vrow + j * 128 + 16);
+                        const double vv[4] = {va.x, va.y, vb.x, vb.y};
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const double ce = v[N + i];
+                            ctr[j][i] = ce;
+#pragma unroll
+                            for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
+                            const double out = fma(w.w[N], ce, acc[PH][j][i]);
+                            if ((int32_t)io[4 * j + i] >= 0) hp[(size_t)io[4 * j + i] * SW_C] = out;
+                            double s = (w0x3 + vv[i]) * ce;
+#pragma unroll
+                            for (int k = 1; k <= N; ++k) {
+                                s = fma(w.w[k], v[N + i + k], s);
+                                s = fma(w.w[k], v[N + i - k], s);
+                            }
+                            acc[PH][j][i] = s;
+                        }
+                    }
+                    // y arms: rows 4py-4 .. 4py+7 of the patch's 4 z columns
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        double u[4 + 2 * N];
+#pragma unroll
+                        for (int tt = 0; tt < 4 + 2 * N; ++tt)
+                            u[tt] = (tt >= N && tt < N + 4) ? ctr[tt - N][i] : pb[((tt - N) * SW_W + N + i) * SW_C];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+#pragma unroll
+                            for (int k = 1; k <= N; ++k) {
+                                acc[PH][j][i] = fma(w.w[k], u[N + j + k], acc[PH][j][i]);
+                                acc[PH][j][i] = fma(w.w[k], u[N + j - k], acc[PH][j][i]);
+                            }
+                    }
+                    // backward half of the x arm: centre values of planes t-1 .. t-4 from tensor memory
+#pragma unroll
+                    for (int k = 1; k <= N; ++k) {
+                        uint32_t pw[32];
+                        tm_ld32(t_in + ((PH + N - k) % N) * 32, pw);
+                        tm_wait_ld32(pw);
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+#pragma unroll
+                            for (int i = 0; i < 4; ++i)
+                                acc[PH][j][i] = fma(w.w[k], __hiloint2double((int)pw[2 * (4 * j + i) + 1], (int)pw[2 * (4 * j + i)]),
+                                                    acc[PH][j][i]);
+                    }
+                } else {
+                    // centre-only plane (warm-up / tail of the work item): it feeds the x arms of its neighbours
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const double ce = pb[(j * SW_W + N + i) * SW_C];
+                            ctr[j][i] = ce;
+#pragma unroll
+                            for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
+                            const double out = fma(w.w[N], ce, acc[PH][j][i]);
+                            if ((int32_t)io[4 * j + i] >= 0) hp[(size_t)io[4 * j + i] * SW_C] = out;
+                            acc[PH][j][i] = 0.0;
+                        }
+                }
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    cw[2 * q] = (uint32_t)__double2loint(ctr[q >> 2][q & 3]);
+                    cw[2 * q + 1] = (uint32_t)__double2hiint(ctr[q >> 2][q & 3]);
+                }
+            } else {
+                // no mesh point of this warp's region in plane t: all centre values are zero
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        if ((int32_t)io[4 * j + i] >= 0) hp[(size_t)io[4 * j + i] * SW_C] = acc[PH][j][i];
+                        acc[PH][j][i] = 0.0;
+                    }
+#pragma unroll
+                for (int q = 0; q < 32; ++q) cw[q] = 0u;
+            }
+            tm_st32(t_in + PH * 32, cw);
+            tm_wait_st();
+
+            hdr_cur = hdr_next;
+            if (++stage == SW_STAGES) {
+                stage = 0;
+                parity ^= 1u;
+            }
+        }
+    }
+    __syncthreads();
+    if (warp == 0)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base_s), "n"(SW_TMEM_COLS) : "memory");
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// host: work items and per-plane records
+// ---------------------------------------------------------------------------------------------
+static int g_max_planes = 32;   // x-slab thickness of a work item (rs_set_tuning("sweep_planes", v))
+void rs_sweep_set_max_planes(int v) { g_max_planes = v < 4 ? 4 : v; }
+
+bool rs_sweep_build_host(const rs_mesh *m, int n, int max_planes, rs_sweep_host &out)
+{
+    if (n != SW_N) return false;
+    const int N = SW_N, T = SW_T, W = SW_W;
     const int nx = m->dims[0], ny = m->dims[1], nz = m->dims[2];
-    const int nrows = ty + 2 * n, w = tz + 2 * n;
-    items.clear();
-    rows.clear();
-    int64_t lanes = 0;
+    out = rs_sweep_host();
     auto point = [&](int x, int y, int z) -> int32_t {
         if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) return -1;
         return m->dense2point[rs_dense_index(m, x, y, z)];
     };
-    for (int y0 = 0; y0 < ny; y0 += ty)
-        for (int z0 = 0; z0 < nz; z0 += tz) {
-            int xlo = nx, xhi = -1;  // planes where the tile interior holds a mesh point
-            for (int x = 0; x < nx; ++x) {
-                bool any = false;
-                for (int y = y0; y < std::min(y0 + ty, ny) && !any; ++y)
-                    for (int z = z0; z < std::min(z0 + tz, nz) && !any; ++z) any = point(x, y, z) >= 0;
-                if (any) {
-                    xlo = std::min(xlo, x);
-                    xhi = std::max(xhi, x);
-                }
-            }
-            if (xhi < xlo) continue;
-            const int len = xhi - xlo + 1;
-            const int nchunks = (len + max_planes - 1) / max_planes;
-            for (int c = 0; c < nchunks; ++c) {
-                rs_sweep_item it;
-                it.y0 = y0;
-                it.z0 = z0;
-                it.xa = xlo + (int)((int64_t)len * c / nchunks);
-                it.xb = xlo + (int)((int64_t)len * (c + 1) / nchunks);
-                it.tab = (int64_t)rows.size();
-                for (int p = it.xa - n; p < it.xb + n; ++p)
-                    for (int r = 0; r < nrows; ++r) {
-                        rs_rowinfo ri = {0, 0, 0};
-                        const int y = y0 - n + r;
-                        const bool halo_row = r < n || r >= ty + n;
-                        for (int zp = halo_row ? n : 0; zp < (halo_row ? n + tz : w); ++zp) {
-                            const int32_t idx = point(p, y, z0 - n + zp);
-                            if (idx < 0) continue;
-                            if (!ri.mask) ri.off = idx;
-                            ri.mask |= (uint64_t)1 << zp;
-                        }
-                        rows.push_back(ri);
+    // planes of each tile that hold a mesh point
+    const int nty = (ny + T - 1) / T, ntz = (nz + T - 1) / T;
+    std::vector<uint8_t> has((size_t)nty * ntz * nx, 0);
+    for (int x = 0; x < nx; ++x)
+        for (int y = 0; y < ny; ++y)
+            for (int z = 0; z < nz; ++z)
+                if (m->dense2point[rs_dense_index(m, x, y, z)] >= 0) has[((size_t)(y / T) * ntz + z / T) * nx + x] = 1;
+
+    for (int xs = 0; xs < nx; xs += max_planes) {            // slab-major: tiles of one slab run together and
+        const int xe = std::min(nx, xs + max_planes);        // find their common halo rows in L2
+        for (int iy = 0; iy < nty; ++iy)
+            for (int iz = 0; iz < ntz; ++iz) {
+                const uint8_t *h = &has[((size_t)iy * ntz + iz) * nx];
+                int xa = -1, xb = -1;
+                for (int x = xs; x < xe; ++x)
+                    if (h[x]) {
+                        if (xa < 0) xa = x;
+                        xb = x + 1;
                     }
-                lanes += (int64_t)(it.xb - it.xa) * ty * tz;
-                items.push_back(it);
-            }
-        }
-    // items that start at the same plane run together: neighbouring tiles then read their common
-    // halo rows at about the same time and find them in L2.
-    std::stable_sort(items.begin(), items.end(),
-                     [](const rs_sweep_item &a, const rs_sweep_item &b) { return a.xa < b.xa; });
-    if (active_lanes) *active_lanes = lanes;
-}
-
-// ---------------------------------------------------------------------------------------------
-// device helpers
-// ---------------------------------------------------------------------------------------------
-template <int VEC>
-struct vec;
-template <>
-struct vec<1> {
-    double x;
-    static __device__ __forceinline__ vec zero() { return {0.0}; }
-    __device__ __forceinline__ void fma(double w, const vec &v) { x = ::fma(w, v.x, x); }
-    static __device__ __forceinline__ vec mul(double w, const vec &v) { return {w * v.x}; }
-};
-template <>
-struct __align__(16) vec<2> {
-    double x, y;
-    static __device__ __forceinline__ vec zero() { return {0.0, 0.0}; }
-    __device__ __forceinline__ void fma(double w, const vec &v)
-    {
-        x = ::fma(w, v.x, x);
-        y = ::fma(w, v.y, y);
-    }
-    static __device__ __forceinline__ vec mul(double w, const vec &v) { return {w * v.x, w * v.y}; }
-};
-
-template <int BYTES>
-__device__ __forceinline__ void cp_async_zfill(void *smem_dst, const void *gsrc, bool valid)
-{
-    const unsigned dst = (unsigned)__cvta_generic_to_shared(smem_dst);
-    const int sz = valid ? BYTES : 0;
-    if constexpr (BYTES == 16)
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(gsrc), "r"(sz) : "memory");
-    else
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(gsrc), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int PENDING>
-__device__ __forceinline__ void cp_async_wait()
-{
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(PENDING) : "memory");
-}
-
-template <int N_, int VEC_, int C_, int TY_, int TZ_, int Q_, int P_, int S_>
-struct sweep_traits {
-    static constexpr int N = N_, VEC = VEC_, C = C_, TY = TY_, TZ = TZ_, Q = Q_, P = P_, S = S_;
-    static constexpr int ROWS = TY + 2 * N, W = TZ + 2 * N;
-    static constexpr int CV = C / VEC;                 // column vectors per point
-    static constexpr int GZ = TZ / P, GY = TY / Q;     // patches per tile row / column
-    static constexpr int THREADS = CV * GZ * GY;
-    static constexpr int WG = W / P;                   // z groups per de-interleaved sub-row
-    static constexpr int PLANE_VECS = ROWS * W * CV;
-    static constexpr int RING = 16;                    // row-record ring (steps t-N .. t+S live)
-    static constexpr size_t SMEM = (size_t)S * PLANE_VECS * VEC * 8 + (size_t)RING * ROWS * sizeof(rs_rowinfo);
-    static constexpr int LOAD_PTS_FULL = TY * W + 2 * N * TZ;
-    static constexpr int LOAD_PTS_CORE = TY * TZ;
-    static_assert(C % VEC == 0 && TZ % P == 0 && TY % Q == 0 && W % P == 0, "tile / patch mismatch");
-    static_assert(W <= 64, "z window must fit one 64-bit occupancy mask");
-    static_assert((CV & (CV - 1)) == 0, "CV must be a power of two");
-    static_assert(N + S < RING, "row-record ring too short");
-    static_assert(THREADS >= ROWS && THREADS <= 1024, "bad thread count");
-};
-
-// shared-memory position (in vec units) of (row r, window position zp, column vector cv): the z axis
-// is de-interleaved by P so that the P-strided patches of adjacent lanes are adjacent in memory.
-template <class T>
-__device__ __forceinline__ int smem_pos(int r, int zp, int cv)
-{
-    return ((r * T::P + zp % T::P) * T::WG + zp / T::P) * T::CV + cv;
-}
-
-template <class T, bool CORE_ONLY>
-__device__ __forceinline__ void load_plane(vec<T::VEC> *stage, const rs_rowinfo *ring_slot, const double *psi,
-                                           int ncol, int col0, int tid)
-{
-    constexpr int NPTS = CORE_ONLY ? T::LOAD_PTS_CORE : T::LOAD_PTS_FULL;
-    constexpr int NEL = NPTS * T::CV;
-#pragma unroll
-    for (int k = 0; k < (NEL + T::THREADS - 1) / T::THREADS; ++k) {
-        const int e = tid + k * T::THREADS;
-        if (e < NEL) {
-            const int pt = e / T::CV, cv = e % T::CV;
-            int r, zp;
-            if (CORE_ONLY) {
-                r = T::N + pt / T::TZ;
-                zp = T::N + pt % T::TZ;
-            } else if (pt < T::TY * T::W) {
-                r = T::N + pt / T::W;
-                zp = pt % T::W;
-            } else {
-                const int q = pt - T::TY * T::W, rr = q / T::TZ;
-                r = rr < T::N ? rr : rr + T::TY;
-                zp = T::N + q % T::TZ;
-            }
-            const rs_rowinfo ri = ring_slot[r];
-            const bool in = (ri.mask >> zp) & 1;
-            const int idx = ri.off + __popcll(ri.mask & (((uint64_t)1 << zp) - 1));
-            const double *src = psi + ((int64_t)(in ? idx : 0) * ncol + col0 + cv * T::VEC);
-            cp_async_zfill<T::VEC * 8>(stage + smem_pos<T>(r, zp, cv), src, in);
-        }
-    }
-}
-
-template <class T>
-__global__ void __launch_bounds__(T::THREADS, 1)
-sweep_kernel(const rs_sweep_item *__restrict__ items, const rs_rowinfo *__restrict__ rows,
-             const double *__restrict__ vloc, const double *__restrict__ psi, double *__restrict__ hpsi, int ncol,
-             int ngroups, const __grid_constant__ rs_weights w)
-{
-    constexpr int N = T::N, Q = T::Q, P = T::P, S = T::S, ROWS = T::ROWS;
-    using V = vec<T::VEC>;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    V *data = reinterpret_cast<V *>(smem_raw);
-    rs_rowinfo *ring = reinterpret_cast<rs_rowinfo *>(smem_raw + (size_t)S * T::PLANE_VECS * sizeof(V));
-
-    const int tid = threadIdx.x;
-    const rs_sweep_item it = items[blockIdx.x / ngroups];
-    const int col0 = (blockIdx.x % ngroups) * T::C;
-    const int steps = (it.xb - it.xa) + 2 * N;     // step t handles lattice plane xa - N + t
-    const rs_rowinfo *tab = rows + it.tab;
-
-    const int cv = tid % T::CV, g = (tid / T::CV) % T::GZ, yq = tid / (T::CV * T::GZ);
-    const int base = ((Q * yq * P) * T::WG + g) * T::CV + cv;   // window corner (row Q*yq, zp P*g) of this thread
-    const int colv = col0 + cv * T::VEC;
-
-    // prologue: row records of steps 0..S-1, then the data of steps 0..S-2
-    for (int e = tid; e < S * ROWS; e += T::THREADS)
-        if (e / ROWS < steps) ring[e] = tab[e];
-    __syncthreads();
-#pragma unroll
-    for (int s = 0; s < S - 1; ++s) {
-        if (s < steps) {
-            if (s < N || s >= steps - N)   // warm-up / tail planes: centre values only, no halo
-                load_plane<T, true>(data + s * T::PLANE_VECS, ring + s * ROWS, psi, ncol, col0, tid);
-            else
-                load_plane<T, false>(data + s * T::PLANE_VECS, ring + s * ROWS, psi, ncol, col0, tid);
-        }
-        cp_async_commit();
-    }
-
-    V in[N][Q][P], acc[N][Q][P];
-#pragma unroll
-    for (int k = 0; k < N; ++k)
-#pragma unroll
-        for (int j = 0; j < Q; ++j)
-#pragma unroll
-            for (int i = 0; i < P; ++i) in[k][j][i] = V::zero(), acc[k][j][i] = V::zero();
-
-    int stage = 0;  // t % S
-    for (int t0 = 0; t0 < steps; t0 += N) {
-#pragma unroll
-        for (int PH = 0; PH < N; ++PH) {
-            const int t = t0 + PH;
-            if (t < steps) {
-                cp_async_wait<S - 2>();
-                __syncthreads();
-                // row record of step t+S (one per thread < ROWS), parked in registers until the end of the step
-                int4 rnext = make_int4(0, 0, 0, 0);
-                const bool fetch = tid < ROWS && t + S < steps;
-                if (fetch) rnext = __ldg(reinterpret_cast<const int4 *>(tab + (int64_t)(t + S) * ROWS + tid));
-                // data of step t+S-1 into the stage that step t-1 has just released
-                {
-                    const int tl = t + S - 1;
-                    if (tl < steps) {
-                        int sl = stage + S - 1;
-                        sl = sl >= S ? sl - S : sl;
-                        V *dst = data + sl * T::PLANE_VECS;
-                        const rs_rowinfo *slot = ring + (tl & (T::RING - 1)) * ROWS;
-                        if (tl < N || tl >= steps - N)
-                            load_plane<T, true>(dst, slot, psi, ncol, col0, tid);
-                        else
-                            load_plane<T, false>(dst, slot, psi, ncol, col0, tid);
-                    }
-                    cp_async_commit();
-                }
-                const V *sp = data + stage * T::PLANE_VECS + base;
-                const bool full = t >= N && t < steps - N;
-                V ctr[Q][P];
-                V a[Q][P];
-                if (full) {
-                    // potential at the thread's own points (latency hidden behind the arm sums)
-                    double vv[Q][P];
-                    const rs_rowinfo *slot = ring + (t & (T::RING - 1)) * ROWS;
-#pragma unroll
-                    for (int j = 0; j < Q; ++j) {
-                        const rs_rowinfo ri = slot[N + Q * yq + j];
-#pragma unroll
-                        for (int i = 0; i < P; ++i) {
-                            const int zp = N + P * g + i;
-                            const bool inb = (ri.mask >> zp) & 1;
-                            const int idx = ri.off + __popcll(ri.mask & (((uint64_t)1 << zp) - 1));
-                            vv[j][i] = inb ? __ldg(vloc + idx) : 0.0;
-                        }
-                    }
-                    // z arms (and the centre values) of the thread's Q rows
-#pragma unroll
-                    for (int j = 0; j < Q; ++j) {
-                        V v[P + 2 * N];
-#pragma unroll
-                        for (int tt = 0; tt < P + 2 * N; ++tt)
-                            v[tt] = sp[(((N + j) * P + tt % P) * T::WG + tt / P) * T::CV];
-#pragma unroll
-                        for (int i = 0; i < P; ++i) {
-                            ctr[j][i] = v[N + i];
-                            V s = V::mul(w.w[1], v[N + i + 1]);
-                            s.fma(w.w[1], v[N + i - 1]);
-#pragma unroll
-                            for (int k = 2; k <= N; ++k) {
-                                s.fma(w.w[k], v[N + i + k]);
-                                s.fma(w.w[k], v[N + i - k]);
-                            }
-                            a[j][i] = s;
-                        }
-                    }
-                    // y arms of the thread's P columns
-#pragma unroll
-                    for (int i = 0; i < P; ++i) {
-                        V u[Q + 2 * N];
-#pragma unroll
-                        for (int tt = 0; tt < Q + 2 * N; ++tt) {
-                            if (tt >= N && tt < N + Q)
-                                u[tt] = ctr[tt - N][i];
-                            else
-                                u[tt] = sp[((tt * P + (N + i) % P) * T::WG + (N + i) / P) * T::CV];
-                        }
-#pragma unroll
-                        for (int j = 0; j < Q; ++j)
-#pragma unroll
-                            for (int k = 1; k <= N; ++k) {
-                                a[j][i].fma(w.w[k], u[N + j + k]);
-                                a[j][i].fma(w.w[k], u[N + j - k]);
-                            }
-                    }
-                    // backward half of the x arm, centre term with the potential
-#pragma unroll
-                    for (int j = 0; j < Q; ++j)
-#pragma unroll
-                        for (int i = 0; i < P; ++i) {
-#pragma unroll
-                            for (int k = 1; k <= N; ++k) a[j][i].fma(w.w[k], in[(PH - k + N) % N][j][i]);
-                            a[j][i].fma(3.0 * w.w[0] + vv[j][i], ctr[j][i]);
-                        }
-                } else {
-#pragma unroll
-                    for (int j = 0; j < Q; ++j)
-#pragma unroll
-                        for (int i = 0; i < P; ++i) {
-                            ctr[j][i] = sp[(((N + j) * P + (N + i) % P) * T::WG + (N + i) / P) * T::CV];
-                            a[j][i] = V::zero();
-                        }
-                }
-                if (t >= N) {
-                    // forward half of the x arm: this plane's centre values feed the n pending outputs
-#pragma unroll
-                    for (int k = 1; k <= N; ++k)
-#pragma unroll
-                        for (int j = 0; j < Q; ++j)
-#pragma unroll
-                            for (int i = 0; i < P; ++i) acc[(PH - k + N) % N][j][i].fma(w.w[k], ctr[j][i]);
-                    if (t >= 2 * N) {
-                        // the output of step t-N is complete
-                        const rs_rowinfo *slot = ring + ((t - N) & (T::RING - 1)) * ROWS;
-#pragma unroll
-                        for (int j = 0; j < Q; ++j) {
-                            const rs_rowinfo ri = slot[N + Q * yq + j];
-#pragma unroll
-                            for (int i = 0; i < P; ++i) {
-                                const int zp = N + P * g + i;
-                                if ((ri.mask >> zp) & 1) {
-                                    const int idx = ri.off + __popcll(ri.mask & (((uint64_t)1 << zp) - 1));
-                                    *reinterpret_cast<V *>(hpsi + ((int64_t)idx * ncol + colv)) = acc[PH][j][i];
+                if (xa < 0) continue;
+                const int y0 = iy * T, z0 = iz * T;
+                const int nsteps = (xb - xa) + 2 * N;
+                out.items.push_back(make_int2((int)out.hdr.size(), nsteps));
+                for (int s = 0; s < nsteps; ++s) {
+                    const int p = xa - N + s;
+                    const bool full = s >= N && s < nsteps - N;
+                    const size_t rec = out.hdr.size();
+                    out.runs.resize((rec + 1) * SW_MAXRUN, make_uint2(0, 0));
+                    out.fill.resize((rec + 1) * 16, 0u);
+                    out.cidx.resize((rec + 1) * 256, -1);
+                    // copy runs and zero-fill bits
+                    int nrun = 0;
+                    auto fill_bit = [&](int e) {   // e: plane slot in loader order (core rows with z halo, then y halo rows)
+                        const int thr = e & 255, which = e >> 8;
+                        out.fill[rec * 16 + (thr >> 4)] |= 1u << (2 * (thr & 15) + which);
+                    };
+                    for (int r = full ? 0 : N; r < (full ? W : N + T); ++r) {
+                        const bool halo_row = r < N || r >= N + T;
+                        const int zlo = (halo_row || !full) ? N : 0, zhi = (halo_row || !full) ? N + T : W;
+                        int run_start = -1;
+                        for (int zp = zlo; zp <= zhi; ++zp) {
+                            const int32_t idx = zp < zhi ? point(p, y0 - N + r, z0 - N + zp) : -1;
+                            if (idx >= 0) {
+                                if (run_start < 0) run_start = zp;
+                            } else {
+                                if (run_start >= 0) {
+                                    if (nrun >= SW_MAXRUN) return false;
+                                    const int32_t first = point(p, y0 - N + r, z0 - N + run_start);
+                                    out.runs[rec * SW_MAXRUN + nrun++] =
+                                        make_uint2((uint32_t)first, (uint32_t)(r * W + run_start) | ((uint32_t)(zp - run_start) << 16));
+                                    run_start = -1;
                                 }
+                                if (zp < zhi) fill_bit(halo_row ? T * W + (r < N ? r : r - T) * T + (zp - N) : (r - N) * W + zp);
                             }
                         }
                     }
-                }
-#pragma unroll
-                for (int j = 0; j < Q; ++j)
-#pragma unroll
-                    for (int i = 0; i < P; ++i) {
-                        acc[PH][j][i] = a[j][i];
-                        in[PH][j][i] = ctr[j][i];
+                    // warp modes and the mesh indices of the tile's own points
+                    uint32_t hdr = 0;
+                    for (int wq = 0; wq < 8; ++wq) {
+                        bool any = false;
+                        for (int y = 4 * (wq >> 1); y < 4 * (wq >> 1) + 4 && !any; ++y)
+                            for (int z = 8 * (wq & 1); z < 8 * (wq & 1) + 8 && !any; ++z) any = point(p, y0 + y, z0 + z) >= 0;
+                        if (any) hdr |= (uint32_t)(full ? MODE_FULL : MODE_CENTRE) << (2 * wq);
                     }
-                if (fetch) reinterpret_cast<int4 *>(ring)[((t + S) & (T::RING - 1)) * ROWS + tid] = rnext;
-                stage = stage + 1 == S ? 0 : stage + 1;
+                    if (full)
+                        for (int y = 0; y < T; ++y)
+                            for (int z = 0; z < T; ++z) out.cidx[rec * 256 + y * T + z] = point(p, y0 + y, z0 + z);
+                    out.hdr.push_back(hdr);
+                }
             }
-        }
     }
-    cp_async_wait<0>();
+    return true;
 }
 
-// ---------------------------------------------------------------------------------------------
-// variants and dispatch
-// ---------------------------------------------------------------------------------------------
-static int g_max_planes = 48;   // x-chunk length of a work item (rs_set_tuning("sweep_planes", v))
-void rs_sweep_set_max_planes(int v) { g_max_planes = v < 8 ? 8 : v; }
+bool rs_sweep_supported(const rs_mesh *m, int n, int ncol)
+{
+    return m->ordering == RS_ORDER_LEX && !m->periodic && n == SW_N && ncol == SW_C;
+}
 
-template <class T>
-static rs_status launch_variant(const rs_mesh *cm, const rs_weights &w, const double *vloc, const double *psi,
-                                double *hpsi, int ncol, cudaStream_t st)
+static rs_status get_tables(rs_mesh *m, int n, const rs_sweep_tables **out)
+{
+    auto f = m->sweep.find(n);
+    if (f == m->sweep.end()) {
+        rs_sweep_host h;
+        rs_sweep_tables tb;
+        tb.ok = rs_sweep_build_host(m, n, g_max_planes, h);
+        if (tb.ok) {
+            tb.nitems = (int64_t)h.items.size();
+            tb.nrec = (int64_t)h.hdr.size();
+            auto up = [&](void **d, const void *src, size_t bytes) -> cudaError_t {
+                cudaError_t e = cudaMalloc(d, bytes);
+                if (e != cudaSuccess) return e;
+                tb.bytes += (int64_t)bytes;
+                return cudaMemcpy(*d, src, bytes, cudaMemcpyHostToDevice);
+            };
+            RS_CUDA_TRY(up((void **)&tb.d_items, h.items.data(), h.items.size() * sizeof(int2)));
+            RS_CUDA_TRY(up((void **)&tb.d_runs, h.runs.data(), h.runs.size() * sizeof(uint2)));
+            RS_CUDA_TRY(up((void **)&tb.d_fill, h.fill.data(), h.fill.size() * sizeof(uint32_t)));
+            RS_CUDA_TRY(up((void **)&tb.d_cidx, h.cidx.data(), h.cidx.size() * sizeof(int32_t)));
+            RS_CUDA_TRY(up((void **)&tb.d_hdr, h.hdr.data(), h.hdr.size() * sizeof(uint32_t)));
+            RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
+        }
+        f = m->sweep.emplace(n, tb).first;
+    }
+    *out = &f->second;
+    return RS_OK;
+}
+
+rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const double *vloc, const double *psi,
+                          double *hpsi, int ncol, cudaStream_t st)
 {
     rs_mesh *m = const_cast<rs_mesh *>(cm);  // lazily filled cache inside the handle
-    const auto key = std::make_tuple(T::N, T::TY, T::TZ);
-    auto f = m->sweep.find(key);
-    if (f == m->sweep.end()) {
-        std::vector<rs_sweep_item> items;
-        std::vector<rs_rowinfo> rows;
-        rs_sweep_tables tb;
-        tb.n = T::N, tb.ty = T::TY, tb.tz = T::TZ;
-        rs_sweep_build_host(m, T::N, T::TY, T::TZ, g_max_planes, items, rows, &tb.active_lanes);
-        tb.nitems = (int64_t)items.size();
-        tb.nrecords = (int64_t)rows.size();
-        RS_CUDA_TRY(cudaMalloc(&tb.d_items, items.size() * sizeof(rs_sweep_item)));
-        RS_CUDA_TRY(cudaMalloc(&tb.d_rows, rows.size() * sizeof(rs_rowinfo)));
-        RS_CUDA_TRY(cudaMemcpy(tb.d_items, items.data(), items.size() * sizeof(rs_sweep_item), cudaMemcpyHostToDevice));
-        RS_CUDA_TRY(cudaMemcpy(tb.d_rows, rows.data(), rows.size() * sizeof(rs_rowinfo), cudaMemcpyHostToDevice));
-        f = m->sweep.emplace(key, tb).first;
-    }
-    static bool attr_set = false;
-    if (!attr_set) {
-        RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM));
-        attr_set = true;
-    }
-    const rs_sweep_tables &tb = f->second;
-    const int ngroups = ncol / T::C;
-    const unsigned grid = (unsigned)(tb.nitems * ngroups);
-    sweep_kernel<T><<<grid, T::THREADS, T::SMEM, st>>>(tb.d_items, tb.d_rows, vloc, psi, hpsi, ncol, ngroups, w);
+    if (!rs_sweep_supported(m, n, ncol)) return rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep kernel cannot serve this call");
+    const rs_sweep_tables *tb = nullptr;
+    rs_status rc = get_tables(m, n, &tb);
+    if (rc != RS_OK) return rc;
+    if (!tb->ok) return rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep tables: a plane needs more copy runs than a record holds");
+    sweep_args a;
+    a.items = tb->d_items, a.runs = tb->d_runs, a.fill = tb->d_fill, a.cidx = tb->d_cidx, a.hdr = tb->d_hdr;
+    a.vloc = vloc, a.psi = psi, a.hpsi = hpsi;
+    sweep_kernel<<<(unsigned)tb->nitems, SW_THREADS, SW_SMEM, st>>>(a, w);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
 }
 
-//                 N  VEC C  TY  TZ  Q  P  S
-// Thread counts are multiples of 128 (one register-file partition per scheduler): 256 threads leave
-// each thread up to 255 registers for its 2n-deep window over a 2 x 2 x VEC patch.
-using sw4_c8 = sweep_traits<4, 2, 8, 16, 16, 2, 2, 3>;
-using sw4_c4 = sweep_traits<4, 2, 4, 16, 32, 2, 2, 3>;
-using sw4_c2 = sweep_traits<4, 2, 2, 32, 32, 2, 2, 3>;
-using sw4_c1 = sweep_traits<4, 1, 1, 32, 32, 2, 2, 3>;
-
-bool rs_sweep_supported(const rs_mesh *m, int n, int ncol)
+// true when the sweep kernel will really serve (mesh, n, ncol): supported and its tables could be built
+bool rs_sweep_usable(const rs_mesh *cm, int n, int ncol)
 {
-    return m->ordering == RS_ORDER_LEX && !m->periodic && n == 4 && ncol >= 1;
+    rs_mesh *m = const_cast<rs_mesh *>(cm);
+    if (!rs_sweep_supported(m, n, ncol) || !m->have_device) return false;
+    const rs_sweep_tables *tb = nullptr;
+    return get_tables(m, n, &tb) == RS_OK && tb->ok;
 }
 
-template <class T>
-static int64_t variant_table_bytes(const rs_mesh *m, int ncol)
+int64_t rs_sweep_table_bytes(const rs_mesh *cm, int n, int ncol)
 {
-    auto f = m->sweep.find(std::make_tuple(T::N, T::TY, T::TZ));
-    if (f == m->sweep.end()) {   // not built yet: build on the host only to count
-        std::vector<rs_sweep_item> items;
-        std::vector<rs_rowinfo> rows;
-        rs_sweep_build_host(m, T::N, T::TY, T::TZ, g_max_planes, items, rows, nullptr);
-        return (int64_t)(rows.size() * sizeof(rs_rowinfo) + items.size() * sizeof(rs_sweep_item)) * (ncol / T::C);
-    }
-    return (f->second.nrecords * (int64_t)sizeof(rs_rowinfo) + f->second.nitems * (int64_t)sizeof(rs_sweep_item)) *
-           (ncol / T::C);
+    rs_mesh *m = const_cast<rs_mesh *>(cm);
+    if (!rs_sweep_supported(m, n, ncol)) return 0;
+    auto f = m->sweep.find(n);
+    if (f != m->sweep.end()) return f->second.bytes;
+    rs_sweep_host h;   // no device (or not built yet): count on the host
+    if (!rs_sweep_build_host(m, n, g_max_planes, h)) return 0;
+    return (int64_t)(h.items.size() * sizeof(int2) + h.runs.size() * sizeof(uint2) + h.fill.size() * 4 + h.cidx.size() * 4 +
+                     h.hdr.size() * 4);
 }
 
-#define RS_SWEEP_DISPATCH(n, ncol, CALL)                      \
-    do {                                                      \
-        if ((n) == 4) {                                       \
-            if ((ncol) >= 8) { CALL(sw4_c8); }                \
-            else if ((ncol) == 4) { CALL(sw4_c4); }           \
-            else if ((ncol) == 2) { CALL(sw4_c2); }           \
-            else { CALL(sw4_c1); }                            \
-        }                                                     \
-    } while (0)
-
-rs_status rs_launch_sweep(const rs_mesh *m, int n, const rs_weights &w, const double *vloc, const double *psi,
-                          double *hpsi, int ncol, cudaStream_t st)
-{
-#define CALL(T) return launch_variant<T>(m, w, vloc, psi, hpsi, ncol, st)
-    RS_SWEEP_DISPATCH(n, ncol, CALL);
-#undef CALL
-    return rs_fail(RS_ERR_UNSUPPORTED, "no plane-sweep variant for this order");
-}
-
-int64_t rs_sweep_table_bytes(const rs_mesh *m, int n, int ncol)
-{
-#define CALL(T) return variant_table_bytes<T>(m, ncol)
-    RS_SWEEP_DISPATCH(n, ncol, CALL);
-#undef CALL
-    return 0;
-}
-
-const char *rs_sweep_variant_name(const rs_mesh *, int n, int ncol)
-{
-    if (n == 4) return ncol >= 8 ? "sweep[n4 c8 16x16 q2p2 s3]" : ncol == 4 ? "sweep[n4 c4 16x32 q2p2 s3]"
-                     : ncol == 2 ? "sweep[n4 c2 32x32 q2p2 s3]" : "sweep[n4 c1 32x32 q2p2 s3]";
-    return "none";
-}
+const char *rs_sweep_variant_name(const rs_mesh *, int, int) { return "sweep[n4 c16 16x16 q4p4 tma+tmem s3]"; }
 
 void rs_sweep_free(rs_mesh *m)
 {
     for (auto &kv : m->sweep) {
-        if (kv.second.d_items) cudaFree(kv.second.d_items);
-        if (kv.second.d_rows) cudaFree(kv.second.d_rows);
+        rs_sweep_tables &t = kv.second;
+        cudaFree(t.d_items), cudaFree(t.d_runs), cudaFree(t.d_fill), cudaFree(t.d_cidx), cudaFree(t.d_hdr);
     }
     m->sweep.clear();
 }
