@@ -24,21 +24,17 @@ constexpr int RS_BRICK_PTS = RS_BRICK * RS_BRICK * RS_BRICK;  // 64 points
 //   cidx[256]              mesh index of the tile's own points (-1: outside the mesh / not an output plane);
 //   hdr                    2 bits per warp: 0 no mesh point in the warp's 4 x 8 region, 1 centre-only, 2 full.
 #define RS_SWEEP_MAXRUN 64
+#define RS_SWEEP_REC_BYTES (RS_SWEEP_MAXRUN * 8 + 64 + 16 + 256 * 4)   // runs | fill | hdr (+pad) | cidx, packed
 struct rs_sweep_host {
-    std::vector<int2> items;      // {first record, number of steps}
-    std::vector<uint2> runs;
-    std::vector<uint32_t> fill;
-    std::vector<int32_t> cidx;
-    std::vector<uint32_t> hdr;
+    std::vector<int2> items;            // {first record, number of steps}
+    std::vector<unsigned char> recs;    // [nrec][RS_SWEEP_REC_BYTES]
+    int64_t nrec = 0;
 };
 struct rs_sweep_tables {
     bool ok = false;              // false: some plane needs more than RS_SWEEP_MAXRUN runs (use the gather kernel)
     int64_t nitems = 0, nrec = 0, bytes = 0;
     int2 *d_items = nullptr;
-    uint2 *d_runs = nullptr;
-    uint32_t *d_fill = nullptr;
-    int32_t *d_cidx = nullptr;
-    uint32_t *d_hdr = nullptr;
+    unsigned char *d_recs = nullptr;
 };
 
 struct rs_mesh {
