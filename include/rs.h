@@ -68,7 +68,7 @@ typedef enum {
     RS_KERNEL_AUTO = 0,   /* best available for this mesh / order / width                         */
     RS_KERNEL_GATHER = 1, /* per-point neighbour table, one gathered load per star arm (any mesh) */
     RS_KERNEL_SWEEP = 2   /* plane-sweep kernel: smem-staged planes + register x-window (RS_ORDER_LEX,
-                             non-periodic mesh, fd_order with a compiled variant)                  */
+                             non-periodic mesh, fd_order 4, 16 | 32 | 64 | 128 real columns)       */
 } rs_kernel;
 
 #define RS_MAX_FD_ORDER 8
@@ -145,9 +145,20 @@ const char *rs_kernel_name(const rs_mesh *mesh, int fd_order, int nst, rs_dtype 
 /* Bytes of neighbour structure the chosen kernel reads per call (for the roofline's algorithmic bytes). */
 int64_t rs_kernel_table_bytes(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, rs_kernel kernel);
 int rs_version(void);
-/* Tuning knobs for tests and ablations (not needed for normal use).  "sweep_planes": x-chunk length of a
- * plane-sweep work item; takes effect for meshes created afterwards.  Unknown name -> RS_ERR_INVALID_ARG. */
+/* Tuning knobs for tests and ablations (not needed for normal use); they take effect for tables built
+ * afterwards.  "sweep_planes": x-slab thickness of a plane-sweep work item (default 32); "sweep_ctas":
+ * number of persistent CTAs (0 = one per SM); "sweep_tensor": 1 = use the 2-D tensor-map copies also for
+ * 16-column blocks.  Unknown name -> RS_ERR_INVALID_ARG.                                               */
 rs_status rs_set_tuning(const char *name, int value);
+/* Host-only diagnostic (no device needed): build the plane-sweep kernel's compact records for (mesh,
+ * fd_order, block width nst of dtype) dealt to `nctas` CTAs with slabs of `max_planes`, replay them
+ * symbolically and verify that they expand to exactly the plain table of rs_mesh_get_index_map and that
+ * every (point, 16-column slice) is produced exactly once (reading S15 of DESIGN.md).  stats_host (may be
+ * NULL) receives {nctas, records, work pieces, modelled cost of the busiest CTA x1000, of the average CTA
+ * x1000, table bytes}.  RS_ERR_UNSUPPORTED if the sweep kernel cannot serve the call; a discrepancy ->
+ * RS_ERR_INVALID_ARG with the first offending (CTA, step, point, arm) in rs_last_error().               */
+rs_status rs_sweep_selfcheck(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, int max_planes, int nctas,
+                             int64_t *stats_host);
 
 #ifdef __cplusplus
 }

@@ -36,6 +36,7 @@ EXPORTS = (
     "rs_mesh_spacing", "rs_mesh_nbricks", "rs_mesh_get_points", "rs_mesh_get_index_map", "rs_block_bytes",
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
     "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version", "rs_set_tuning",
+    "rs_sweep_selfcheck",
 )
 
 
@@ -80,6 +81,7 @@ def _load() -> C.CDLL:
     L.rs_kernel_table_bytes.restype = C.c_int64
     L.rs_version.restype = C.c_int
     L.rs_set_tuning.argtypes = [C.c_char_p, C.c_int]
+    L.rs_sweep_selfcheck.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]
     return L
 
 
@@ -165,6 +167,14 @@ def rs_version() -> int:
 
 def rs_set_tuning(name: str, value: int) -> None:
     _check(_lib.rs_set_tuning(name.encode(), value))
+
+
+def rs_sweep_selfcheck(mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, max_planes: int = 32, nctas: int = 148) -> dict:
+    """Host-only replay of the plane-sweep records against the plain neighbour table; raises on a discrepancy."""
+    st = (C.c_int64 * 6)()
+    _check(_lib.rs_sweep_selfcheck(mesh.handle, fd_order, nst, dtype, max_planes, nctas, st))
+    return {"nctas": st[0], "records": st[1], "pieces": st[2], "cost_max": st[3] / 1000.0, "cost_mean": st[4] / 1000.0,
+            "table_bytes": st[5]}
 
 
 def rs_mesh_create(centers, radius: float, spacing: float, max_fd_order: int = 4,

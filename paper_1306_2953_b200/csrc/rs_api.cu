@@ -144,11 +144,35 @@ extern "C" rs_status rs_hamiltonian_apply_states_host(const rs_mesh *m, int n, c
 }
 
 void rs_sweep_set_max_planes(int v);
+void rs_sweep_set_force_tensor(int v);
+void rs_sweep_set_nctas(int v);
+std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, int64_t *stats);
+
 extern "C" rs_status rs_set_tuning(const char *name, int value)
 {
     if (name && std::strcmp(name, "sweep_planes") == 0) {
         rs_sweep_set_max_planes(value);
         return RS_OK;
     }
+    if (name && std::strcmp(name, "sweep_tensor") == 0) {
+        rs_sweep_set_force_tensor(value);
+        return RS_OK;
+    }
+    if (name && std::strcmp(name, "sweep_ctas") == 0) {
+        rs_sweep_set_nctas(value);
+        return RS_OK;
+    }
     return rs_fail(RS_ERR_INVALID_ARG, "rs_set_tuning: unknown knob");
+}
+
+extern "C" rs_status rs_sweep_selfcheck(const rs_mesh *m, int n, int nst, rs_dtype dtype, int max_planes, int nctas,
+                                        int64_t *stats_host)
+{
+    if (!m || nst < 1 || max_planes < 4 || nctas < 1 || (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_sweep_selfcheck: bad argument");
+    const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
+    const std::string msg = rs_sweep_selfcheck_host(m, n, ncol, max_planes, nctas, stats_host);
+    if (msg.rfind("unsupported", 0) == 0) return rs_fail(RS_ERR_UNSUPPORTED, msg);
+    if (!msg.empty()) return rs_fail(RS_ERR_INVALID_ARG, "plane-sweep records: " + msg);
+    return RS_OK;
 }

@@ -15,20 +15,28 @@ constexpr int RS_BRICK_PTS = RS_BRICK * RS_BRICK * RS_BRICK;  // 64 points
 
 // ---- plane-sweep kernel tables (rs_sweep.cu) -------------------------------------------------------
 // The compact form of the neighbour table ("a compact form of it is used"; reading S15):
-// one record per (work item, lattice plane).  A work item is a 16 x 16 tile of the (y, z) plane and a
-// range [xa, xb) of x planes; its steps cover planes xa-4 .. xb+3 (the first and last 4 only feed the
-// x arms).  A record holds
-//   runs[RS_SWEEP_MAXRUN]  {first mesh index, destination slot | npoints << 16}: one bulk copy per run of
+// one record per (CTA, step).  A CTA's steps walk through its work pieces; a piece is a 16 x 16 tile of
+// the (y, z) plane, a range [xa, xb) of x planes and a 16-column slice of the block; its steps cover
+// planes xa-4 .. xb+3 (the first and last 4 only feed the x arms).  A record holds
+//   runs[RS_SWEEP_MAXRUN]  {first mesh index, destination slot | npoints << 16}: one copy per run of
 //                          consecutive in-domain points of a z-row (consecutive in memory in RS_ORDER_LEX);
-//   fill[16]               2 bits per thread: zero-fill its two plane slots (lattice point outside the mesh);
-//   cidx[256]              mesh index of the tile's own points (-1: outside the mesh / not an output plane);
-//   hdr                    2 bits per warp: 0 no mesh point in the warp's 4 x 8 region, 1 centre-only, 2 full.
+//   fill[18 (+2 pad)]      bitmap over the stage's [24][24] slots: slots to clear (lattice point outside the mesh
+//                          and the stage buffer does not already hold zeros there);
+//   hdr[4]                 {2 bits per warp: 0 no mesh point in the warp's 4 x 8 region, 1 centre-only, 2 full;
+//                           bit 16: output plane,  column offset of the slice,  bytes copied (1-D runs),
+//                           bytes copied (2-D tensor boxes)};
+//   cidx[256]              mesh index of the tile's own points (-1: outside the mesh / not an output plane).
 #define RS_SWEEP_MAXRUN 64
-#define RS_SWEEP_REC_BYTES (RS_SWEEP_MAXRUN * 8 + 64 + 16 + 256 * 4)   // runs | fill | hdr (+pad) | cidx, packed
+#define RS_SWEEP_REC_BYTES (RS_SWEEP_MAXRUN * 8 + 80 + 16 + 256 * 4)   // runs | fill | hdr | cidx, packed
+struct rs_sweep_piece {
+    int iy, iz, xa, xb, chunk;   // tile, output planes [xa, xb), column slice
+};
 struct rs_sweep_host {
-    std::vector<int2> items;            // {first record, number of steps}
-    std::vector<unsigned char> recs;    // [nrec][RS_SWEEP_REC_BYTES]
+    std::vector<int2> items;                         // per CTA: {first record, number of steps}
+    std::vector<std::vector<rs_sweep_piece>> pieces; // per CTA, in execution order
+    std::vector<unsigned char> recs;                 // [nrec][RS_SWEEP_REC_BYTES]
     int64_t nrec = 0;
+    double cost_max = 0.0, cost_mean = 0.0;          // modelled load of the busiest / average CTA
 };
 struct rs_sweep_tables {
     bool ok = false;              // false: some plane needs more than RS_SWEEP_MAXRUN runs (use the gather kernel)
@@ -57,7 +65,7 @@ struct rs_mesh {
     int device = -1;
     int sm_count = 0;
     int32_t *d_map[RS_MAX_FD_ORDER + 1] = {nullptr};                 // [np][6n], built lazily per order
-    std::map<int, rs_sweep_tables> sweep;                            // fd_order -> tables, built lazily
+    std::map<std::pair<int, int>, rs_sweep_tables> sweep;            // (fd_order, ncol) -> tables, built lazily
 };
 
 void rs_set_error(const std::string &msg);
@@ -98,4 +106,4 @@ int64_t rs_sweep_table_bytes(const rs_mesh *m, int n, int ncol);
 const char *rs_sweep_variant_name(const rs_mesh *m, int n, int ncol);
 void rs_sweep_free(rs_mesh *m);
 // host-only construction of the records; false if a plane needs more than RS_SWEEP_MAXRUN runs
-bool rs_sweep_build_host(const rs_mesh *m, int n, int max_planes, rs_sweep_host &out);
+bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out);

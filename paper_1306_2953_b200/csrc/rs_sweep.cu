@@ -1,31 +1,42 @@
 // Plane-sweep kernel: the fused stencil + local potential (step a5; eq. 2 :41)
-// as a 2.5-D streaming kernel written for sm_100a (TMA bulk copies, mbarriers, tensor memory).
+// as a persistent, warp-specialised 2.5-D streaming kernel for sm_100a (TMA copies, mbarriers,
+// tensor memory, setmaxnreg).
 //
 // What differs from the paper's kernel (one thread per (point, orbital), every star arm
 // a separate load through a neighbour table) and why -- see DESIGN.md "Kernels":
-//   * A CTA owns a 16 x 16 tile of the lattice's (y, z) plane and 16 block columns, and marches along
-//     x.  Plane p of the tile plus its y/z halos (no corners) is staged in shared memory ONCE by
-//     bulk async copies (cp.async.bulk, one per run of in-domain points of a z-row: such a run is
-//     one contiguous span of the blocked array because the orbital index is fastest);
-//     completion is tracked by an mbarrier per stage.  Lattice points outside the mesh are zero-filled
-//     in shared memory (reading S3), so the compute code has no predicates.
-//   * A thread owns a 4 x 4 patch of (y, z) points of ONE column (the 16 lanes of a half-warp are the
+//   * One CTA per SM, persistent.  The host cuts the mesh into work items (a 16 x 16 tile of the
+//     lattice's (y, z) plane x a slab of x planes x 16 block columns), orders them slab by slab (so
+//     that tiles sharing halo rows run at about the same time and find them in L2) and deals them
+//     to the CTAs with a cost model, splitting items in x where needed so that all CTAs finish together.
+//     A CTA marches through its items plane by plane.
+//   * Producer warp: stages plane p of the tile plus its y/z halo strips (no corners) in shared
+//     memory ONCE, by bulk async copies -- one per run of in-domain points of a z-row: such a run
+//     is one contiguous span of the blocked array because the orbital index is fastest;
+//     for blocks wider than 16 columns the CTA takes a 16-column slice and the same runs become 2-D
+//     tensor-map copies.  Completion is tracked by an mbarrier per stage (3 stages).  Lattice points
+//     outside the mesh are zero-filled in shared memory (reading S3), so the arithmetic has no
+//     predicates.  The producer also gathers V and the mesh indices of the tile's 256 points.
+//   * 8 consumer warps, no block-wide barrier: they wait on the stage's "full" mbarrier and release it
+//     through an "empty" mbarrier, so warps drift by up to two planes and hide each other's stalls.
+//     A thread owns a 4 x 4 patch of (y, z) points of ONE column (the 16 lanes of a half-warp are the
 //     16 columns of a point: every shared-memory read is a conflict-free 128-byte row).  The y/z arm
 //     operands are shared inside the patch: 5 shared-memory reads per output instead of 17.
 //   * The x arm never touches shared memory: the forward half is accumulated into the 4 pending
 //     outputs of each (y, z) column held in registers; the backward half needs the centre values of
 //     the previous 4 planes, which are parked in TENSOR MEMORY (tcgen05.st / tcgen05.ld, 32x32b shape:
-//     every thread owns one TMEM lane, i.e. a private 2 KB scratch with ~2.6x the bandwidth of shared
-//     memory, measured).  No tensor-core arithmetic is involved: the path is not a contraction.
-//   * The neighbour table is replaced by per-(tile, plane) records built once on the host: the list of
+//     every thread owns one TMEM lane, a private scratch).  No tensor-core arithmetic is involved:
+//     the path is not a contraction.
+//   * The neighbour table is replaced by per-(item, plane) records built once on the host: the list of
 //     copy runs, zero-fill bits, the mesh index of each of the tile's 256 points (for V and for the
 //     store) and a 2-bit mode per warp (empty / centre-only / full) that lets a warp skip the planes
 //     in which its 4 x 8 region holds no mesh point.  The records expand to exactly the plain table of
-//     rs_mesh_get_index_map (reading S15).
+//     rs_mesh_get_index_map (reading S15; rs_sweep_selfcheck verifies this on the host).
 // Requires RS_ORDER_LEX (in-domain points of a z-row consecutive in memory), a non-periodic mesh,
-// fd_order 4 and a block of 16 real columns (B = 16 real or B = 8 complex); anything else is served by
-// the gather kernel.
+// fd_order 4 and a block of 16, 32, 64 or 128 real columns; anything else is served by the gather kernel.
+#include <cuda.h>
+
 #include <algorithm>
+#include <cstring>
 
 #include "rs_internal.h"
 
@@ -36,17 +47,24 @@ constexpr int SW_T = 16;                 // tile edge (points) in y and z
 constexpr int SW_W = SW_T + 2 * SW_N;    // 24: rows / z-slots of a staged plane
 constexpr int SW_C = 16;                 // columns per CTA
 constexpr int SW_SLOT_BYTES = SW_C * 8;  // 128
-constexpr int SW_STAGE_BYTES = SW_W * SW_W * SW_SLOT_BYTES;  // 73,728: uniform [24][24] slots, corners hold V and idx
+constexpr int SW_STAGE_BYTES = SW_W * SW_W * SW_SLOT_BYTES;  // 73,728: uniform [24][24] slots; corners hold V, idx, header
 constexpr int SW_STAGES = 3;
-constexpr int SW_THREADS = 256;
+constexpr int SW_CONSUMERS = 256;        // 8 consumer warps
+constexpr int SW_THREADS = 384;          // + one producer warpgroup
 constexpr int SW_MAXRUN = RS_SWEEP_MAXRUN;
-constexpr int SW_TMEM_COLS = 512;        // allocated; used: 2 x (4 x 32 [centre ring] + 4 x 16 [index ring])
-// packed per-plane record (rs_internal.h): runs | fill bits | header | indices of the tile's points
-constexpr int SW_REC_RUNS = 0, SW_REC_FILL = SW_MAXRUN * 8, SW_REC_HDR = SW_REC_FILL + 64, SW_REC_CIDX = SW_REC_HDR + 16;
+constexpr int SW_TMEM_COLS = 512;        // allocated; used: 2 x (4 x 32 [centre ring] + 4 x 16 [offset ring])
+// packed per-plane record (rs_internal.h): runs | fill rows | header | indices of the tile's points
+constexpr int SW_REC_RUNS = 0, SW_REC_FILL = SW_MAXRUN * 8, SW_REC_HDR = SW_REC_FILL + 80, SW_REC_CIDX = SW_REC_HDR + 16;
 constexpr int SW_REC_BYTES = RS_SWEEP_REC_BYTES;
 static_assert(SW_REC_BYTES == SW_REC_CIDX + 256 * 4 && SW_REC_BYTES % 16 == 0, "record layout");
-constexpr int SW_RING = 4;               // record ring: record r is requested 3 steps before it is consumed
+constexpr int SW_RING = 6;               // record ring of the producer group
+constexpr int SW_LOOKAHEAD = 3;          // records are requested this many steps ahead (SW_RING >= SW_LOOKAHEAD + 3)
 constexpr size_t SW_SMEM = (size_t)SW_STAGES * SW_STAGE_BYTES + (size_t)SW_RING * SW_REC_BYTES;
+static_assert(SW_SMEM + 256 <= 232448, "shared memory budget");
+constexpr int SW_NBOX = 6;               // tensor-map box heights 1, 2, 4, 8, 16, 24
+
+enum { MODE_EMPTY = 0, MODE_CENTRE = 1, MODE_FULL = 2 };
+constexpr uint32_t HDR_OUTPUT_PLANE = 1u << 16;   // the plane has outputs: stage V and the indices
 
 // ---------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -60,6 +78,14 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.expect_tx.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
@@ -82,22 +108,21 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
-__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const void *src, uint32_t src_bytes)
+// 2-D tensor-map copy: box {16 columns, box rows} at (column c0, row c1) -> shared, rows packed 128 B apart
+__device__ __forceinline__ void tensor_g2s(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar)
 {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async_arrive_noinc(uint32_t bar)
-{
-    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
 }
-
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 // ---- tensor memory: every thread reads / writes consecutive 32-bit columns of its own lane -------
@@ -154,127 +179,133 @@ __device__ __forceinline__ double words2double(uint32_t lo, uint32_t hi) { retur
 // the kernel
 // ---------------------------------------------------------------------------------------------
 struct sweep_args {
-    const int2 *items;           // {first record, number of steps}
+    const int2 *items;           // per CTA: {first record, number of steps}
     const unsigned char *recs;   // [nrec][SW_REC_BYTES] packed per-plane records
     const double *vloc;
     const double *psi;
     double *hpsi;
+    uint32_t ncol;               // row pitch of the block in elements
+};
+struct sweep_maps {
+    CUtensorMap box[SW_NBOX];    // psi as a [np+1][ncol] fp64 tensor, box {16, 1|2|4|8|16|24}
 };
 
-enum { MODE_EMPTY = 0, MODE_CENTRE = 1, MODE_FULL = 2 };
-constexpr uint32_t HDR_OUTPUT_PLANE = 1u << 16;   // the plane has outputs: stage V and the indices
+// stage offsets of the small per-plane arrays kept in the unused corners of the [24][24] slot grid
+constexpr uint32_t SW_HDR_OFF = (uint32_t)((SW_W - SW_N) * SW_W) * SW_SLOT_BYTES;   // corner C: row 20, slot 0
 
-__global__ void __launch_bounds__(SW_THREADS, 1)
-sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_weights w)
+// ---- producer warpgroup (4 warps): stage plane after plane --------------------------------------------
+// Every warp takes a quarter of each job (copy runs, zero fill, V / index gather) and arrives once on the
+// stage's "full" barrier.  Records arrive through a ring of SW_RING slots, requested SW_LOOKAHEAD steps
+// ahead by thread 0: a warp working on step t proves that all warps finished step t - 3 (the consumers
+// released that stage), so the slot of record t - 3 = slot of record t + 3 may be overwritten.
+template <bool TENSOR>
+__device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_maps &maps, unsigned char *smem,
+                                               uint32_t full0, uint32_t empty0, uint32_t rbar0, const unsigned char *recs,
+                                               int nsteps, int ptid)
 {
     constexpr int N = SW_N;
-    extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ uint64_t full_bar[SW_STAGES];
-    __shared__ uint64_t rec_bar[SW_RING];
-    __shared__ uint32_t tmem_base_s;
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int c = tid & 15, patch = tid >> 4, py = patch >> 2, pz = patch & 3;
-    const int2 item = a.items[blockIdx.x];
-    const unsigned char *const recs = a.recs + (size_t)item.x * SW_REC_BYTES;
-    const int nsteps = item.y;
-
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < SW_STAGES; ++s) mbar_init(smem_u32(&full_bar[s]), SW_THREADS);
-#pragma unroll
-        for (int s = 0; s < SW_RING; ++s) mbar_init(smem_u32(&rec_bar[s]), 1);
-        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-    }
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_base_s)),
-                     "n"(SW_TMEM_COLS)
-                     : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    // this thread's TMEM lane (its warp's quarter) and the column range of its warp
-    const uint32_t tbase = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(warp >> 2) * 192u;
-    const uint32_t t_in = tbase;          // [patch row j][slot t mod 4][i]: centre values of the last 4 planes (doubles)
-    const uint32_t t_ix = tbase + 128u;   // [slot t mod 4][16]: mesh indices of the last 4 planes' outputs
-
-    const uint32_t sbase = smem_u32(smem);
-    const uint32_t bar0 = smem_u32(&full_bar[0]);
-    const uint32_t rbar0 = smem_u32(&rec_bar[0]);
+    const int lane = ptid & 31, pw = ptid >> 5;
     unsigned char *const ring = smem + (size_t)SW_STAGES * SW_STAGE_BYTES;
-
-    // ---- loader constants: two plane slots to zero-fill, one tile point for V and the index ----------
-    uint32_t fill_off1, fill_off2;
-    {
-        const int e1 = tid, e2 = tid + 256;
-        fill_off1 = (uint32_t)(((N + e1 / SW_W) * SW_W + e1 % SW_W) * SW_SLOT_BYTES);
-        if (e2 < SW_T * SW_W)
-            fill_off2 = (uint32_t)(((N + e2 / SW_W) * SW_W + e2 % SW_W) * SW_SLOT_BYTES);
-        else {
-            const int q = e2 - SW_T * SW_W, hr = q / SW_T;
-            fill_off2 = (uint32_t)((((hr < N ? hr : hr + SW_T)) * SW_W + N + q % SW_T) * SW_SLOT_BYTES);
+    const uint32_t sbase = smem_u32(smem);
+    auto request_rec = [&](int r) {   // thread 0
+        const uint32_t bar = rbar0 + 8u * (r % SW_RING);
+        fence_proxy_async();
+        mbar_arrive_expect_tx(bar, SW_REC_BYTES);
+        bulk_g2s(smem_u32(ring) + (uint32_t)(r % SW_RING) * SW_REC_BYTES, recs + (size_t)r * SW_REC_BYTES, SW_REC_BYTES, bar);
+    };
+    if (ptid == 0)
+        for (int r = 0; r < SW_LOOKAHEAD && r < nsteps; ++r) request_rec(r);
+    // this thread's jobs: copy run `myrun` (lanes 0..15 of each warp), fill slots ptid + 128 k, tile points ptid and ptid + 128
+    const int myrun = lane * 4 + pw;
+    int stage = 0, rs = 0;
+    uint32_t eparity = 1, rparity = 0;   // the first pass over the stages finds them free
+    for (int t = 0; t < nsteps; ++t) {
+        mbar_wait(empty0 + 8u * stage, eparity);
+        mbar_wait(rbar0 + 8u * rs, rparity);
+        const unsigned char *rp = ring + (size_t)rs * SW_REC_BYTES;
+        const uint32_t sb = sbase + (uint32_t)stage * SW_STAGE_BYTES;
+        unsigned char *const sg = smem + (size_t)stage * SW_STAGE_BYTES;
+        const uint32_t bar = full0 + 8u * stage;
+        const uint4 hdr = *reinterpret_cast<const uint4 *>(rp + SW_REC_HDR);   // {modes|flags, column offset, tx bytes 1-D, tx bytes 2-D}
+        if (ptid == 0) {
+            mbar_expect_tx(bar, TENSOR ? hdr.w : hdr.z);
+            *reinterpret_cast<uint2 *>(sg + SW_HDR_OFF) = make_uint2(hdr.x, hdr.y);
+        }
+        // ---- copy runs --------------------------------------------------------------------------------
+        if (lane < SW_MAXRUN / 4) {
+            const uint2 r = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
+            const uint32_t len = r.y >> 16, slot = r.y & 0xffffu;
+            if (len) {
+                if constexpr (!TENSOR) {
+                    bulk_g2s(sb + slot * SW_SLOT_BYTES, a.psi + (size_t)r.x * SW_C, len * SW_SLOT_BYTES, bar);
+                } else {
+                    // largest box height (1, 2, 4, 8, 16 or 24) not above len; a second, overlapping box covers the rest
+                    const int lg = len >= 24 ? 5 : 31 - __clz((int)len);
+                    const uint32_t p = len >= 24 ? 24u : 1u << lg;
+                    tensor_g2s(sb + slot * SW_SLOT_BYTES, &maps.box[lg], (int)hdr.y, (int)r.x, bar);
+                    if (p < len)
+                        tensor_g2s(sb + (slot + len - p) * SW_SLOT_BYTES, &maps.box[lg], (int)hdr.y, (int)(r.x + len - p), bar);
+                }
+            }
+        }
+        // ---- zero fill: bit s of the record's bitmap says that slot s of the [24][24] grid must be cleared ----
+#pragma unroll
+        for (int k = 0; k < (SW_W * SW_W + 127) / 128; ++k) {
+            const int sl = ptid + 128 * k;
+            if (sl < SW_W * SW_W) {
+                const uint32_t m = *reinterpret_cast<const uint32_t *>(rp + SW_REC_FILL + (sl >> 5) * 4);
+                if ((m >> (sl & 31)) & 1u) {
+                    float4 *d = reinterpret_cast<float4 *>(sg + (size_t)sl * SW_SLOT_BYTES);
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) d[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+            }
+        }
+        // ---- V and the mesh indices of the tile's own points (output planes only) ----------------------
+        if (hdr.x & HDR_OUTPUT_PLANE) {
+            int32_t ci[2];
+            double vv[2];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) ci[q] = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + (ptid + 128 * q) * 4);
+#pragma unroll
+            for (int q = 0; q < 2; ++q) vv[q] = ci[q] >= 0 ? __ldg(a.vloc + ci[q]) : 0.0;
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const int p = ptid + 128 * q, ty = p >> 4, tz = p & 15;
+                *reinterpret_cast<double *>(sg + ((ty >> 2) * SW_W) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 8) = vv[q];
+                *reinterpret_cast<int32_t *>(sg + ((ty >> 2) * SW_W + SW_W - N) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 4) = ci[q];
+            }
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar);
+        if (ptid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
+        if (++stage == SW_STAGES) {
+            stage = 0;
+            eparity ^= 1u;
+        }
+        if (++rs == SW_RING) {
+            rs = 0;
+            rparity ^= 1u;
         }
     }
-    const int ty = tid >> 4, tz = tid & 15;
-    // corner A (rows 0..3, slots 0..3) holds V[16][16]; corner B (rows 0..3, slots 20..23) holds idx[16][16]
-    const uint32_t v_off = (uint32_t)(((ty >> 2) * SW_W) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 8);
-    const uint32_t i_off = (uint32_t)(((ty >> 2) * SW_W + SW_W - N) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 4);
-    // ---- compute constants -------------------------------------------------------------------------
+}
+
+// ---- consumer warps: the arithmetic ----------------------------------------------------------------
+__device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_weights &w, const unsigned char *smem,
+                                               uint32_t full0, uint32_t empty0, uint32_t tmem_base, int nsteps, int tid)
+{
+    constexpr int N = SW_N;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int c = tid & 15, patch = tid >> 4, py = patch >> 2, pz = patch & 3;
+    // this thread's TMEM lane (its warp's quarter) and the column range of its warp
+    const uint32_t tbase = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(warp >> 2) * 192u;
+    const uint32_t t_in = tbase;          // [patch row j][slot t mod 4][i]: centre values of the last 4 planes (doubles)
+    const uint32_t t_ix = tbase + 128u;   // [slot t mod 4][16]: store offsets of the last 4 planes' outputs
+
     const uint32_t b0 = (uint32_t)(((N + 4 * py) * SW_W + 4 * pz) * SW_SLOT_BYTES + c * 8);   // patch row 0, window slot 0
     const uint32_t vrow = (uint32_t)((py * SW_W) * SW_SLOT_BYTES + (4 * pz) * 8);
     const uint32_t irow = (uint32_t)((py * SW_W + SW_W - N) * SW_SLOT_BYTES + (4 * pz) * 4);
-
-    // ---- record ring: record r lands in slot r mod 4, two steps before produce(r) reads it ----------------
-    auto request_rec = [&](int r) {   // one thread
-        const uint32_t bar = rbar0 + 8u * (r & (SW_RING - 1));
-        fence_proxy_async();
-        mbar_arrive_expect_tx(bar, SW_REC_BYTES);
-        bulk_g2s(smem_u32(ring) + (uint32_t)(r & (SW_RING - 1)) * SW_REC_BYTES, recs + (size_t)r * SW_REC_BYTES, SW_REC_BYTES, bar);
-    };
-    // ---- producer: stage plane tl; returns the plane's header word ------------------------------------
-    auto produce = [&](int tl, int stage_l) -> uint32_t {
-        const int rs = tl & (SW_RING - 1);
-        mbar_wait(rbar0 + 8u * rs, (uint32_t)(tl >> 2) & 1u);
-        const unsigned char *rp = ring + (size_t)rs * SW_REC_BYTES;
-        const uint32_t sb = sbase + (uint32_t)stage_l * SW_STAGE_BYTES;
-        unsigned char *const sg = smem + (size_t)stage_l * SW_STAGE_BYTES;
-        const uint32_t bar = bar0 + 8u * stage_l;
-        if (warp == 0) {
-            const uint2 r0 = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + lane * 8);
-            const uint2 r1 = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + 256 + lane * 8);
-            const uint32_t n0 = r0.y >> 16, n1 = r1.y >> 16;
-            fence_proxy_async();
-            if (n0 + n1) mbar_expect_tx(bar, (n0 + n1) * SW_SLOT_BYTES);
-            if (n0) bulk_g2s(sb + (r0.y & 0xffffu) * SW_SLOT_BYTES, a.psi + (size_t)r0.x * SW_C, n0 * SW_SLOT_BYTES, bar);
-            if (n1) bulk_g2s(sb + (r1.y & 0xffffu) * SW_SLOT_BYTES, a.psi + (size_t)r1.x * SW_C, n1 * SW_SLOT_BYTES, bar);
-        }
-        const uint32_t hdr = *reinterpret_cast<const uint32_t *>(rp + SW_REC_HDR);
-        const uint32_t fb = *reinterpret_cast<const uint32_t *>(rp + SW_REC_FILL + (tid >> 4) * 4) >> (2 * (tid & 15));
-        if (fb & 1u) {
-            float4 *d = reinterpret_cast<float4 *>(sg + fill_off1);
-#pragma unroll
-            for (int q = 0; q < 8; ++q) d[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-        if (fb & 2u) {
-            float4 *d = reinterpret_cast<float4 *>(sg + fill_off2);
-#pragma unroll
-            for (int q = 0; q < 8; ++q) d[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-        if (hdr & HDR_OUTPUT_PLANE) {
-            const int32_t ci = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + tid * 4);
-            *reinterpret_cast<int32_t *>(sg + i_off) = ci;
-            if (ci >= 0) cp_async8_zfill(sb + v_off, a.vloc + ci, 8u);
-        }
-        cp_async_arrive_noinc(bar);
-        return hdr;
-    };
-
-    if (tid == 0)
-        for (int r = 0; r < SW_RING && r < nsteps; ++r) request_rec(r);
-    uint32_t hdr_a = produce(0, 0);                 // nsteps >= 2 N + 1
-    uint32_t hdr_b = produce(1, 1);
 
     double acc[N][4][4];   // pending outputs: acc[t mod 4] belongs to plane t
 #pragma unroll
@@ -283,6 +314,13 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
         for (int j = 0; j < 4; ++j)
 #pragma unroll
             for (int i = 0; i < 4; ++i) acc[k][j][i] = 0.0;
+    {   // no pending output yet: all parked offsets invalid
+        uint32_t inv[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) inv[q] = 0xffffffffu;
+#pragma unroll
+        for (int k = 0; k < N; ++k) tm_st16(t_ix + k * 16, inv);
+    }
 
     int stage = 0;
     uint32_t parity = 0;
@@ -294,26 +332,25 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
         for (int PH = 0; PH < N; ++PH) {
             const int t = t0 + PH;
             if (t >= nsteps) break;
-            // mesh indices of the outputs this step completes (plane t - 4); in flight during the barrier
+            // store offsets of the outputs this step completes (plane t - 4); in flight during the wait
             tm_wait_st();
             uint32_t io[16];
             tm_ld16(t_ix + PH * 16, io);
-            mbar_wait(bar0 + 8u * stage, parity);
-            __syncthreads();
-            if (tid == 0 && t + SW_RING < nsteps) request_rec(t + SW_RING);
-            uint32_t hdr_c = 0;
-            if (t + SW_STAGES - 1 < nsteps) hdr_c = produce(t + SW_STAGES - 1, stage == 0 ? SW_STAGES - 1 : stage - 1);
-            const int mode = (int)((hdr_a >> (2 * warp)) & 3u);
+            mbar_wait(full0 + 8u * stage, parity);
             const unsigned char *sp = smem + (size_t)stage * SW_STAGE_BYTES;
+            const uint2 hdr = *reinterpret_cast<const uint2 *>(sp + SW_HDR_OFF);   // {modes | flags, column offset}
+            const int mode = (int)((hdr.x >> (2 * warp)) & 3u);
             const double *pb = reinterpret_cast<const double *>(sp + b0);
 
-            uint32_t in_[16];   // this plane's output indices, parked for 4 steps
+            uint32_t in_[16];   // this plane's store offsets, parked for 4 steps
             if (mode == MODE_FULL) {
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int4 q = *reinterpret_cast<const int4 *>(sp + irow + j * 64);
-                    in_[4 * j] = (uint32_t)q.x, in_[4 * j + 1] = (uint32_t)q.y, in_[4 * j + 2] = (uint32_t)q.z,
-                            in_[4 * j + 3] = (uint32_t)q.w;
+                    const int qq[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        in_[4 * j + i] = qq[i] >= 0 ? (uint32_t)qq[i] * a.ncol + hdr.y : 0xffffffffu;
                 }
             } else {
 #pragma unroll
@@ -342,7 +379,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
 #pragma unroll
                         for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
                         const double out = fma(w.w[N], ce, acc[PH][j][i]);
-                        if ((int32_t)io[4 * j + i] >= 0) hp[(size_t)io[4 * j + i] * SW_C] = out;
+                        if (io[4 * j + i] != 0xffffffffu) hp[io[4 * j + i]] = out;
                         s[i] = (w0x3 + vv[i]) * ce;
 #pragma unroll
                         for (int k = 1; k <= N; ++k) {
@@ -385,7 +422,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
                         }
                 }
             } else if (mode == MODE_CENTRE) {
-                // centre-only plane (warm-up / tail of the work item): it feeds the x arms of its neighbours
+                // centre-only plane (warm-up / tail of a work item): it feeds the x arms of its neighbours
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     uint32_t cw[8];
@@ -395,7 +432,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
 #pragma unroll
                         for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
                         const double out = fma(w.w[N], ce, acc[PH][j][i]);
-                        if ((int32_t)io[4 * j + i] >= 0) hp[(size_t)io[4 * j + i] * SW_C] = out;
+                        if (io[4 * j + i] != 0xffffffffu) hp[io[4 * j + i]] = out;
                         acc[PH][j][i] = 0.0;
                         cw[2 * i] = (uint32_t)__double2loint(ce);
                         cw[2 * i + 1] = (uint32_t)__double2hiint(ce);
@@ -411,15 +448,15 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
                 for (int j = 0; j < 4; ++j) {
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
-                        if ((int32_t)io[4 * j + i] >= 0) hp[(size_t)io[4 * j + i] * SW_C] = acc[PH][j][i];
+                        if (io[4 * j + i] != 0xffffffffu) hp[io[4 * j + i]] = acc[PH][j][i];
                         acc[PH][j][i] = 0.0;
                     }
                     tm_st8(t_in + j * 32 + PH * 8, cw);
                 }
             }
-
-            hdr_a = hdr_b;
-            hdr_b = hdr_c;
+            // this warp has read everything it needs from the stage
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8u * stage);
             if (++stage == SW_STAGES) {
                 stage = 0;
                 parity ^= 1u;
@@ -427,142 +464,364 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
         }
     }
     tm_wait_st();
+}
+
+template <bool TENSOR>
+__global__ void __launch_bounds__(SW_THREADS, 1)
+sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_weights w, const __grid_constant__ sweep_maps maps)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ uint64_t full_bar[SW_STAGES];
+    __shared__ uint64_t empty_bar[SW_STAGES];
+    __shared__ uint64_t rec_bar[SW_RING];
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const int2 item = a.items[blockIdx.x];
+    const int nsteps = item.y;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < SW_STAGES; ++s) {
+            mbar_init(smem_u32(&full_bar[s]), (SW_THREADS - SW_CONSUMERS) / 32);
+            mbar_init(smem_u32(&empty_bar[s]), SW_CONSUMERS / 32);
+        }
+#pragma unroll
+        for (int s = 0; s < SW_RING; ++s) mbar_init(smem_u32(&rec_bar[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_base_s)),
+                     "n"(SW_TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __syncthreads();
-    if (warp == 0)
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base_s), "n"(SW_TMEM_COLS) : "memory");
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+
+    // register re-split: 384 x 168 at launch = 128 x 40 (producer group) + 256 x 232 (consumers); the pool that
+    // setmaxnreg.inc draws from holds only what setmaxnreg.dec released, so the two must balance exactly
+    if (tid >= SW_CONSUMERS) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
+        sweep_producer<TENSOR>(a, maps, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), smem_u32(&rec_bar[0]),
+                               a.recs + (size_t)item.x * SW_REC_BYTES, nsteps, tid - SW_CONSUMERS);
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
+        sweep_consumer(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, tid);
+        named_bar_sync(1, SW_CONSUMERS);
+        if (warp == 0)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base_s), "n"(SW_TMEM_COLS) : "memory");
+    }
 }
 
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
-// host: work items and per-plane records
+// host: work pieces, their assignment to CTAs, and the per-step records
 // ---------------------------------------------------------------------------------------------
 static int g_max_planes = 32;   // x-slab thickness of a work item (rs_set_tuning("sweep_planes", v))
+static int g_force_tensor = 0;  // rs_set_tuning("sweep_tensor", 1): use the tensor-map copies also for 16 columns (tests)
+static int g_nctas = 0;         // rs_set_tuning("sweep_ctas", v): persistent CTAs (0 = one per SM)
 void rs_sweep_set_max_planes(int v) { g_max_planes = v < 4 ? 4 : v; }
+void rs_sweep_set_force_tensor(int v) { g_force_tensor = v != 0; }
+void rs_sweep_set_nctas(int v) { g_nctas = v < 0 ? 0 : v; }
 
-bool rs_sweep_build_host(const rs_mesh *m, int n, int max_planes, rs_sweep_host &out)
-{
-    if (n != SW_N) return false;
-    const int N = SW_N, T = SW_T, W = SW_W;
-    const int nx = m->dims[0], ny = m->dims[1], nz = m->dims[2];
-    out = rs_sweep_host();
-    auto point = [&](int x, int y, int z) -> int32_t {
+namespace {
+
+// modelled cost of one consumer-warp step by mode (relative to a full step), and of a whole step:
+// warps w and w + 4 share a scheduler, the busiest scheduler paces the step
+constexpr double COST_MODE[3] = {0.04, 0.15, 1.0};
+constexpr double COST_STEP_FIXED = 0.05;
+
+struct tile_geometry {
+    const rs_mesh *m;
+    int nx, ny, nz, nty, ntz;
+    int32_t point(int x, int y, int z) const
+    {
         if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) return -1;
         return m->dense2point[rs_dense_index(m, x, y, z)];
-    };
-    // planes of each tile that hold a mesh point
-    const int nty = (ny + T - 1) / T, ntz = (nz + T - 1) / T;
-    std::vector<uint8_t> has((size_t)nty * ntz * nx, 0);
-    for (int x = 0; x < nx; ++x)
-        for (int y = 0; y < ny; ++y)
-            for (int z = 0; z < nz; ++z)
-                if (m->dense2point[rs_dense_index(m, x, y, z)] >= 0) has[((size_t)(y / T) * ntz + z / T) * nx + x] = 1;
+    }
+    // 2 bits per warp for plane x of tile (iy, iz): which warps' 4 x 8 regions hold a mesh point
+    uint32_t warp_modes(int iy, int iz, int x, int mode) const
+    {
+        uint32_t hdr = 0;
+        for (int wq = 0; wq < 8; ++wq) {
+            bool any = false;
+            for (int y = 4 * (wq >> 1); y < 4 * (wq >> 1) + 4 && !any; ++y)
+                for (int z = 8 * (wq & 1); z < 8 * (wq & 1) + 8 && !any; ++z) any = point(x, iy * SW_T + y, iz * SW_T + z) >= 0;
+            if (any) hdr |= (uint32_t)mode << (2 * wq);
+        }
+        return hdr;
+    }
+};
 
+double step_cost(uint32_t modes)
+{
+    double worst = 0.0;
+    for (int q = 0; q < 4; ++q) {
+        const double c = COST_MODE[(modes >> (2 * q)) & 3u] + COST_MODE[(modes >> (2 * (q + 4))) & 3u];
+        worst = std::max(worst, c);
+    }
+    return COST_STEP_FIXED + 0.5 * worst;
+}
+
+}  // namespace
+
+bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out)
+{
+    if (n != SW_N || ncol % SW_C != 0 || nctas < 1) return false;
+    const int N = SW_N, T = SW_T, W = SW_W;
+    tile_geometry g{m, m->dims[0], m->dims[1], m->dims[2], (m->dims[1] + T - 1) / T, (m->dims[2] + T - 1) / T};
+    const int nx = g.nx, nchunks = ncol / SW_C;
+    out = rs_sweep_host();
+
+    // ---- cost of every (tile, plane) as a full step; 0 where the tile has no mesh point in the plane ----
+    std::vector<double> fcost((size_t)g.nty * g.ntz * nx, 0.0), ccost((size_t)g.nty * g.ntz * nx, 0.0);
+    for (int iy = 0; iy < g.nty; ++iy)
+        for (int iz = 0; iz < g.ntz; ++iz)
+            for (int x = 0; x < nx; ++x) {
+                const uint32_t mf = g.warp_modes(iy, iz, x, MODE_FULL);
+                if (mf) {
+                    fcost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(mf);
+                    ccost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(g.warp_modes(iy, iz, x, MODE_CENTRE));
+                }
+            }
+    auto halo_cost = [&](int iy, int iz, int xa, int xb) {   // the 2 N centre-only steps around [xa, xb)
+        double c = 0.0;
+        const double *cc = &ccost[((size_t)iy * g.ntz + iz) * nx];
+        for (int k = 1; k <= N; ++k) {
+            c += (xa - k >= 0 && cc[xa - k] > 0.0) ? cc[xa - k] : COST_STEP_FIXED + 0.5 * 2 * COST_MODE[MODE_EMPTY];
+            c += (xb + k - 1 < nx && cc[xb + k - 1] > 0.0) ? cc[xb + k - 1] : COST_STEP_FIXED + 0.5 * 2 * COST_MODE[MODE_EMPTY];
+        }
+        return c;
+    };
+    auto range_cost = [&](int iy, int iz, int xa, int xb) {
+        double c = 0.0;
+        const double *fc = &fcost[((size_t)iy * g.ntz + iz) * nx];
+        for (int x = xa; x < xb; ++x) c += fc[x] > 0.0 ? fc[x] : COST_STEP_FIXED + 0.5 * 2 * COST_MODE[MODE_EMPTY];
+        return c;
+    };
+
+    // ---- work items in execution order: slab by slab, column slice by column slice, tile by tile -------
+    std::vector<rs_sweep_piece> items;
+    double total = 0.0;
+    for (int xs = 0; xs < nx; xs += max_planes) {
+        const int xe = std::min(nx, xs + max_planes);
+        for (int ch = 0; ch < nchunks; ++ch)
+            for (int iy = 0; iy < g.nty; ++iy)
+                for (int iz = 0; iz < g.ntz; ++iz) {
+                    const double *fc = &fcost[((size_t)iy * g.ntz + iz) * nx];
+                    int xa = -1, xb = -1;
+                    for (int x = xs; x < xe; ++x)
+                        if (fc[x] > 0.0) {
+                            if (xa < 0) xa = x;
+                            xb = x + 1;
+                        }
+                    if (xa < 0) continue;
+                    items.push_back({iy, iz, xa, xb, ch});
+                    total += range_cost(iy, iz, xa, xb) + halo_cost(iy, iz, xa, xb);
+                }
+    }
+    // ---- deal them out: always to the least-loaded CTA; an item that would overshoot the common finish
+    //      line is split in x, the rest goes back to the head of the queue ---------------------------------
+    std::vector<double> load;
+    auto deal = [&](double finish, std::vector<std::vector<rs_sweep_piece>> &pieces) -> double {
+        pieces.assign(nctas, {});
+        load.assign(nctas, 0.0);
+        std::vector<char> closed(nctas, 0);   // CTAs that cannot take another piece without overshooting
+        const int MIN_SPLIT = 6;              // output planes: below this the 2 N halo steps dominate
+        auto least_loaded = [&](bool open_only) {
+            int best = -1;
+            for (int c = 0; c < nctas; ++c)
+                if ((!open_only || !closed[c]) && (best < 0 || load[c] < load[best])) best = c;
+            return best;
+        };
+        for (size_t q = 0; q < items.size(); ++q) {
+            rs_sweep_piece it = items[q];
+            for (;;) {
+                int cta = least_loaded(true);
+                const double whole = range_cost(it.iy, it.iz, it.xa, it.xb) + halo_cost(it.iy, it.iz, it.xa, it.xb);
+                if (cta < 0) {   // every CTA is at the finish line: the least loaded takes the overshoot
+                    cta = least_loaded(false);
+                    pieces[cta].push_back(it);
+                    load[cta] += whole;
+                    break;
+                }
+                if (load[cta] + whole <= finish) {
+                    pieces[cta].push_back(it);
+                    load[cta] += whole;
+                    break;
+                }
+                // largest prefix [xa, xsplit) that still fits, leaving at least MIN_SPLIT planes on either side
+                int xsplit = it.xa;
+                double c = halo_cost(it.iy, it.iz, it.xa, it.xb);
+                const double *fc = &fcost[((size_t)it.iy * g.ntz + it.iz) * nx];
+                while (xsplit < it.xb - MIN_SPLIT) {
+                    const double cx = fc[xsplit] > 0.0 ? fc[xsplit] : COST_STEP_FIXED + COST_MODE[MODE_EMPTY];
+                    if (load[cta] + c + cx > finish) break;
+                    c += cx;
+                    ++xsplit;
+                }
+                if (xsplit - it.xa < MIN_SPLIT) {
+                    closed[cta] = 1;
+                    continue;
+                }
+                rs_sweep_piece head = it;
+                head.xb = xsplit;
+                pieces[cta].push_back(head);
+                load[cta] += range_cost(head.iy, head.iz, head.xa, head.xb) + halo_cost(head.iy, head.iz, head.xa, head.xb);
+                it.xa = xsplit;
+            }
+        }
+        return *std::max_element(load.begin(), load.end());
+    };
+    // the lowest common finish line that the dealing meets without overshoot (bisection)
+    double lo = total / nctas, hi = lo * 1.05 + 2.0;
+    std::vector<std::vector<rs_sweep_piece>> trial;
+    while (deal(hi, trial) > hi) hi = hi * 1.25 + 2.0;
+    for (int it = 0; it < 14; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (deal(mid, trial) <= mid)
+            hi = mid;
+        else
+            lo = mid;
+    }
+    deal(hi, out.pieces);
+    for (double l : load) {
+        out.cost_max = std::max(out.cost_max, l);
+        out.cost_mean += l / nctas;
+    }
+
+    // ---- records: one per (CTA, step) ----------------------------------------------------------------
     enum { UNKNOWN = 0, ZERO = 1, DATA = 2 };
     std::vector<uint8_t> state((size_t)SW_STAGES * W * W);
-    for (int xs = 0; xs < nx; xs += max_planes) {            // slab-major: tiles of one slab run together and
-        const int xe = std::min(nx, xs + max_planes);        // find their common halo rows in L2
-        for (int iy = 0; iy < nty; ++iy)
-            for (int iz = 0; iz < ntz; ++iz) {
-                const uint8_t *h = &has[((size_t)iy * ntz + iz) * nx];
-                int xa = -1, xb = -1;
-                for (int x = xs; x < xe; ++x)
-                    if (h[x]) {
-                        if (xa < 0) xa = x;
-                        xb = x + 1;
-                    }
-                if (xa < 0) continue;
-                const int y0 = iy * T, z0 = iz * T;
-                const int nsteps = (xb - xa) + 2 * N;
-                out.items.push_back(make_int2((int)out.nrec, nsteps));
-                std::fill(state.begin(), state.end(), (uint8_t)UNKNOWN);   // shared memory of a starting CTA is arbitrary
-                for (int s = 0; s < nsteps; ++s) {
-                    const int p = xa - N + s;
-                    const bool full = s >= N && s < nsteps - N;
-                    out.recs.resize((size_t)(out.nrec + 1) * SW_REC_BYTES, 0);
-                    unsigned char *rec = out.recs.data() + (size_t)out.nrec * SW_REC_BYTES;
-                    uint2 *runs = reinterpret_cast<uint2 *>(rec + SW_REC_RUNS);
-                    uint32_t *fill = reinterpret_cast<uint32_t *>(rec + SW_REC_FILL);
-                    uint32_t *hdrp = reinterpret_cast<uint32_t *>(rec + SW_REC_HDR);
-                    int32_t *cidx = reinterpret_cast<int32_t *>(rec + SW_REC_CIDX);
-                    uint8_t *st = &state[(size_t)(s % SW_STAGES) * W * W];
-                    // copy runs, and zero-fill bits for the slots this plane reads that are outside the mesh and
-                    // do not already hold zeros from an earlier plane staged in the same buffer
-                    int nrun = 0;
-                    auto fill_bit = [&](int e) {   // e: plane slot in loader order (core rows with z halo, then y halo rows)
-                        const int thr = e & 255, which = e >> 8;
-                        fill[thr >> 4] |= 1u << (2 * (thr & 15) + which);
-                    };
-                    for (int r = full ? 0 : N; r < (full ? W : N + T); ++r) {
-                        const bool halo_row = r < N || r >= N + T;
-                        const int zlo = (halo_row || !full) ? N : 0, zhi = (halo_row || !full) ? N + T : W;
-                        int run_start = -1;
-                        for (int zp = zlo; zp <= zhi; ++zp) {
-                            const int32_t idx = zp < zhi ? point(p, y0 - N + r, z0 - N + zp) : -1;
-                            if (idx >= 0) {
-                                if (run_start < 0) run_start = zp;
-                                st[r * W + zp] = DATA;
-                            } else {
-                                if (run_start >= 0) {
-                                    if (nrun >= SW_MAXRUN) return false;
-                                    const int32_t first = point(p, y0 - N + r, z0 - N + run_start);
-                                    runs[nrun++] = make_uint2((uint32_t)first,
-                                                              (uint32_t)(r * W + run_start) | ((uint32_t)(zp - run_start) << 16));
-                                    run_start = -1;
-                                }
-                                if (zp < zhi && st[r * W + zp] != ZERO) {
-                                    fill_bit(halo_row ? T * W + (r < N ? r : r - T) * T + (zp - N) : (r - N) * W + zp);
-                                    st[r * W + zp] = ZERO;
-                                }
+    out.items.resize(nctas);
+    for (int cta = 0; cta < nctas; ++cta) {
+        std::fill(state.begin(), state.end(), (uint8_t)UNKNOWN);   // shared memory of a starting CTA is arbitrary
+        const int64_t first = out.nrec;
+        int step = 0;                                               // stage of a step = step mod SW_STAGES, as in the kernel
+        for (const rs_sweep_piece &pc : out.pieces[cta]) {
+            const int y0 = pc.iy * T, z0 = pc.iz * T;
+            const int nsteps = (pc.xb - pc.xa) + 2 * N;
+            for (int s = 0; s < nsteps; ++s, ++step) {
+                const int p = pc.xa - N + s;
+                const bool full = s >= N && s < nsteps - N;
+                out.recs.resize((size_t)(out.nrec + 1) * SW_REC_BYTES, 0);
+                unsigned char *rec = out.recs.data() + (size_t)out.nrec * SW_REC_BYTES;
+                uint2 *runs = reinterpret_cast<uint2 *>(rec + SW_REC_RUNS);
+                uint32_t *fill = reinterpret_cast<uint32_t *>(rec + SW_REC_FILL);
+                uint32_t *hdrp = reinterpret_cast<uint32_t *>(rec + SW_REC_HDR);
+                int32_t *cidx = reinterpret_cast<int32_t *>(rec + SW_REC_CIDX);
+                uint8_t *st = &state[(size_t)(step % SW_STAGES) * W * W];
+                // copy runs, and zero-fill bits for the slots this plane reads that are outside the mesh and
+                // do not already hold zeros from an earlier plane staged in the same buffer
+                int nrun = 0;
+                uint32_t tx1 = 0, tx2 = 0;
+                for (int r = full ? 0 : N; r < (full ? W : N + T); ++r) {
+                    const bool halo_row = r < N || r >= N + T;
+                    const int zlo = (halo_row || !full) ? N : 0, zhi = (halo_row || !full) ? N + T : W;
+                    int run_start = -1;
+                    for (int zp = zlo; zp <= zhi; ++zp) {
+                        const int32_t idx = zp < zhi ? g.point(p, y0 - N + r, z0 - N + zp) : -1;
+                        if (idx >= 0) {
+                            if (run_start < 0) run_start = zp;
+                            st[r * W + zp] = DATA;
+                        } else {
+                            if (run_start >= 0) {
+                                if (nrun >= SW_MAXRUN) return false;
+                                const int32_t firstp = g.point(p, y0 - N + r, z0 - N + run_start);
+                                const uint32_t len = (uint32_t)(zp - run_start);
+                                runs[nrun++] = make_uint2((uint32_t)firstp, (uint32_t)(r * W + run_start) | (len << 16));
+                                uint32_t box = 24;
+                                if (len < 24)
+                                    for (box = 1; box * 2 <= len; box *= 2) {}
+                                tx1 += len * SW_SLOT_BYTES;
+                                tx2 += (box < len ? 2 * box : box) * SW_SLOT_BYTES;
+                                run_start = -1;
+                            }
+                            if (zp < zhi && st[r * W + zp] != ZERO) {
+                                fill[(r * W + zp) >> 5] |= 1u << ((r * W + zp) & 31);
+                                st[r * W + zp] = ZERO;
                             }
                         }
                     }
-                    // warp modes and the mesh indices of the tile's own points
-                    uint32_t hdr = full ? HDR_OUTPUT_PLANE : 0u;
-                    for (int wq = 0; wq < 8; ++wq) {
-                        bool any = false;
-                        for (int y = 4 * (wq >> 1); y < 4 * (wq >> 1) + 4 && !any; ++y)
-                            for (int z = 8 * (wq & 1); z < 8 * (wq & 1) + 8 && !any; ++z) any = point(p, y0 + y, z0 + z) >= 0;
-                        if (any) hdr |= (uint32_t)(full ? MODE_FULL : MODE_CENTRE) << (2 * wq);
-                    }
-                    for (int y = 0; y < T; ++y)
-                        for (int z = 0; z < T; ++z) cidx[y * T + z] = full ? point(p, y0 + y, z0 + z) : -1;
-                    *hdrp = hdr;
-                    ++out.nrec;
                 }
+                hdrp[0] = g.warp_modes(pc.iy, pc.iz, p, full ? MODE_FULL : MODE_CENTRE) | (full ? HDR_OUTPUT_PLANE : 0u);
+                hdrp[1] = (uint32_t)(pc.chunk * SW_C);
+                hdrp[2] = tx1;
+                hdrp[3] = tx2;
+                for (int y = 0; y < T; ++y)
+                    for (int z = 0; z < T; ++z) cidx[y * T + z] = full ? g.point(p, y0 + y, z0 + z) : -1;
+                ++out.nrec;
             }
+        }
+        out.items[cta] = make_int2((int)first, step);
     }
     return true;
 }
 
 bool rs_sweep_supported(const rs_mesh *m, int n, int ncol)
 {
-    return m->ordering == RS_ORDER_LEX && !m->periodic && n == SW_N && ncol == SW_C;
+    return m->ordering == RS_ORDER_LEX && !m->periodic && n == SW_N && ncol >= SW_C && ncol % SW_C == 0 &&
+           (uint64_t)(m->np + 1) * (uint64_t)ncol < 0xffffffffull;   // store offsets are 32-bit element offsets
 }
 
-static rs_status get_tables(rs_mesh *m, int n, const rs_sweep_tables **out)
+static int sweep_nctas(const rs_mesh *m) { return g_nctas > 0 ? g_nctas : (m->sm_count > 0 ? m->sm_count : 148); }
+
+static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables **out)
 {
-    auto f = m->sweep.find(n);
+    const auto key = std::make_pair(n, ncol);
+    auto f = m->sweep.find(key);
     if (f == m->sweep.end()) {
         rs_sweep_host h;
         rs_sweep_tables tb;
-        tb.ok = rs_sweep_build_host(m, n, g_max_planes, h);
+        tb.ok = rs_sweep_build_host(m, n, ncol, g_max_planes, sweep_nctas(m), h);
         if (tb.ok) {
             tb.nitems = (int64_t)h.items.size();
             tb.nrec = h.nrec;
             auto up = [&](void **d, const void *src, size_t bytes) -> cudaError_t {
-                cudaError_t e = cudaMalloc(d, bytes);
-                if (e != cudaSuccess) return e;
+                cudaError_t e = cudaMalloc(d, bytes ? bytes : 16);
+                if (e != cudaSuccess || bytes == 0) return e;
                 tb.bytes += (int64_t)bytes;
                 return cudaMemcpy(*d, src, bytes, cudaMemcpyHostToDevice);
             };
             RS_CUDA_TRY(up((void **)&tb.d_items, h.items.data(), h.items.size() * sizeof(int2)));
             RS_CUDA_TRY(up((void **)&tb.d_recs, h.recs.data(), h.recs.size()));
-            RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
+            RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
+            RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
         }
-        f = m->sweep.emplace(n, tb).first;
+        f = m->sweep.emplace(key, tb).first;
     }
     *out = &f->second;
+    return RS_OK;
+}
+
+// psi viewed as a [np + 1][ncol] fp64 tensor; one map per box height (1, 2, 4, 8, 16, 24 rows x 16 columns)
+static rs_status encode_maps(const rs_mesh *m, const double *psi, int ncol, sweep_maps &maps)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        RS_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) return rs_fail(RS_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+        encode = (encode_fn)fn;
+    }
+    static const cuuint32_t heights[SW_NBOX] = {1, 2, 4, 8, 16, 24};
+    const cuuint64_t dims[2] = {(cuuint64_t)ncol, (cuuint64_t)(m->np + 1)};
+    const cuuint64_t strides[1] = {(cuuint64_t)ncol * 8};
+    const cuuint32_t estr[2] = {1, 1};
+    for (int b = 0; b < SW_NBOX; ++b) {
+        const cuuint32_t box[2] = {(cuuint32_t)SW_C, heights[b]};
+        const CUresult r = encode(&maps.box[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(psi), dims, strides, box,
+                                  estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return rs_fail(RS_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    }
     return RS_OK;
 }
 
@@ -572,13 +831,23 @@ rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const d
     rs_mesh *m = const_cast<rs_mesh *>(cm);  // lazily filled cache inside the handle
     if (!rs_sweep_supported(m, n, ncol)) return rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep kernel cannot serve this call");
     const rs_sweep_tables *tb = nullptr;
-    rs_status rc = get_tables(m, n, &tb);
+    rs_status rc = get_tables(m, n, ncol, &tb);
     if (rc != RS_OK) return rc;
     if (!tb->ok) return rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep tables: a plane needs more copy runs than a record holds");
     sweep_args a;
     a.items = tb->d_items, a.recs = tb->d_recs;
-    a.vloc = vloc, a.psi = psi, a.hpsi = hpsi;
-    sweep_kernel<<<(unsigned)tb->nitems, SW_THREADS, SW_SMEM, st>>>(a, w);
+    a.vloc = vloc, a.psi = psi, a.hpsi = hpsi, a.ncol = (uint32_t)ncol;
+    sweep_maps maps;
+    const bool tensor = ncol != SW_C || g_force_tensor;
+    if (tensor) {
+        if (((uintptr_t)psi & 15u) != 0) return rs_fail(RS_ERR_INVALID_ARG, "psi must be 16-byte aligned");
+        rc = encode_maps(m, psi, ncol, maps);
+        if (rc != RS_OK) return rc;
+        sweep_kernel<true><<<(unsigned)tb->nitems, SW_THREADS, SW_SMEM, st>>>(a, w, maps);
+    } else {
+        std::memset(&maps, 0, sizeof(maps));
+        sweep_kernel<false><<<(unsigned)tb->nitems, SW_THREADS, SW_SMEM, st>>>(a, w, maps);
+    }
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
 }
@@ -589,21 +858,25 @@ bool rs_sweep_usable(const rs_mesh *cm, int n, int ncol)
     rs_mesh *m = const_cast<rs_mesh *>(cm);
     if (!rs_sweep_supported(m, n, ncol) || !m->have_device) return false;
     const rs_sweep_tables *tb = nullptr;
-    return get_tables(m, n, &tb) == RS_OK && tb->ok;
+    return get_tables(m, n, ncol, &tb) == RS_OK && tb->ok;
 }
 
 int64_t rs_sweep_table_bytes(const rs_mesh *cm, int n, int ncol)
 {
     rs_mesh *m = const_cast<rs_mesh *>(cm);
     if (!rs_sweep_supported(m, n, ncol)) return 0;
-    auto f = m->sweep.find(n);
+    auto f = m->sweep.find(std::make_pair(n, ncol));
     if (f != m->sweep.end()) return f->second.bytes;
     rs_sweep_host h;   // no device (or not built yet): count on the host
-    if (!rs_sweep_build_host(m, n, g_max_planes, h)) return 0;
+    if (!rs_sweep_build_host(m, n, ncol, g_max_planes, sweep_nctas(m), h)) return 0;
     return (int64_t)(h.items.size() * sizeof(int2) + h.recs.size());
 }
 
-const char *rs_sweep_variant_name(const rs_mesh *, int, int) { return "sweep[n4 c16 16x16 q4p4 tma+tmem s3]"; }
+const char *rs_sweep_variant_name(const rs_mesh *, int, int ncol)
+{
+    return (ncol != SW_C || g_force_tensor) ? "sweep[n4 c16 16x16 q4p4 persistent ws tma2d+tmem s3]"
+                                            : "sweep[n4 c16 16x16 q4p4 persistent ws tma1d+tmem s3]";
+}
 
 void rs_sweep_free(rs_mesh *m)
 {
@@ -612,4 +885,109 @@ void rs_sweep_free(rs_mesh *m)
         cudaFree(t.d_items), cudaFree(t.d_recs);
     }
     m->sweep.clear();
+}
+
+// ---------------------------------------------------------------------------------------------
+// host self-check: replay the records symbolically (mesh indices instead of values) exactly as the
+// kernel consumes them and verify that every output point sees, arm by arm, the neighbours that the
+// plain table of rs_mesh_get_index_map names (reading S15), and that every (point, column slice) is
+// produced exactly once.  Returns an empty string on success, else the first discrepancy.
+// ---------------------------------------------------------------------------------------------
+std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, int64_t *stats)
+{
+    if (!rs_sweep_supported(m, n, ncol)) return "unsupported (ordering / order / width)";
+    rs_sweep_host h;
+    if (!rs_sweep_build_host(m, n, ncol, max_planes, nctas, h)) return "a plane needs more copy runs than a record holds";
+    const int N = SW_N, T = SW_T, W = SW_W, NS = 6 * N;
+    const int64_t np = m->np;
+    std::vector<int32_t> map((size_t)np * NS);
+    rs_build_index_map(m, n, map.data());
+    auto arm = [&](int32_t ip, int axis, int k) -> int32_t {   // k != 0; returns -1 for the zero slot
+        const int32_t v = map[(size_t)ip * NS + axis * 2 * N + 2 * (std::abs(k) - 1) + (k > 0 ? 0 : 1)];
+        return v == np ? -1 : v;
+    };
+    const int nchunks = ncol / SW_C;
+    std::vector<uint8_t> done((size_t)np * nchunks, 0);
+    int64_t npieces = 0;
+    auto fail = [&](int cta, int step, const char *what, int y, int z, int k) {
+        return std::string(what) + " (cta " + std::to_string(cta) + ", step " + std::to_string(step) + ", y " + std::to_string(y) +
+               ", z " + std::to_string(z) + ", k " + std::to_string(k) + ")";
+    };
+    const int32_t UNK = -2;
+    for (int cta = 0; cta < nctas; ++cta) {
+        npieces += (int64_t)h.pieces[cta].size();
+        std::vector<int32_t> stage((size_t)SW_STAGES * W * W, UNK);
+        // per tile point: centre values seen at the last 4 steps and the outputs pending from them
+        std::vector<int32_t> hist((size_t)T * T * N, UNK), pend((size_t)T * T * N, -1), pend_chunk((size_t)T * T * N, 0);
+        const int nsteps = h.items[cta].y;
+        for (int t = 0; t < nsteps; ++t) {
+            const unsigned char *rec = h.recs.data() + (size_t)(h.items[cta].x + t) * SW_REC_BYTES;
+            const uint2 *runs = reinterpret_cast<const uint2 *>(rec + SW_REC_RUNS);
+            const uint32_t *fill = reinterpret_cast<const uint32_t *>(rec + SW_REC_FILL);
+            const uint32_t *hdr = reinterpret_cast<const uint32_t *>(rec + SW_REC_HDR);
+            const int32_t *cidx = reinterpret_cast<const int32_t *>(rec + SW_REC_CIDX);
+            int32_t *sg = &stage[(size_t)(t % SW_STAGES) * W * W];
+            uint32_t tx1 = 0;
+            for (int r = 0; r < SW_MAXRUN; ++r) {
+                const uint32_t len = runs[r].y >> 16, slot = runs[r].y & 0xffffu;
+                if (slot + len > (uint32_t)(W * W)) return fail(cta, t, "run leaves the stage", 0, 0, r);
+                for (uint32_t i = 0; i < len; ++i) sg[slot + i] = (int32_t)(runs[r].x + i);
+                tx1 += len * SW_SLOT_BYTES;
+            }
+            if (tx1 != hdr[2]) return fail(cta, t, "byte count of the copy runs", 0, 0, 0);
+            for (int r = 0; r < W; ++r)
+                for (int z = 0; z < W; ++z)
+                    if ((fill[(r * W + z) >> 5] >> ((r * W + z) & 31)) & 1u) sg[r * W + z] = -1;
+            const int chunk = (int)hdr[1] / SW_C;
+            const int ph = t % N;
+            for (int y = 0; y < T; ++y)
+                for (int z = 0; z < T; ++z) {
+                    const int wq = (y / 4) * 2 + z / 8;
+                    const int mode = (int)((hdr[0] >> (2 * wq)) & 3u);
+                    const int32_t ci = (hdr[0] & HDR_OUTPUT_PLANE) ? cidx[y * T + z] : -1;
+                    int32_t *hp = &hist[(size_t)(y * T + z) * N], *pp = &pend[(size_t)(y * T + z) * N];
+                    int32_t *pc = &pend_chunk[(size_t)(y * T + z) * N];
+                    const int32_t ce = mode == MODE_EMPTY ? -1 : sg[(N + y) * W + N + z];
+                    // forward half of the x arm of the outputs pending from the last 4 steps
+                    for (int k = 1; k <= N; ++k) {
+                        const int32_t o = pp[(ph + N - k) % N];
+                        if (k < N ? o >= 0 : false)
+                            if (arm(o, 0, k) != ce) return fail(cta, t, "forward x arm", y, z, k);
+                    }
+                    {   // the output of plane t - 4 completes now
+                        const int32_t o = pp[ph];
+                        if (o >= 0) {
+                            if (arm(o, 0, N) != ce) return fail(cta, t, "forward x arm", y, z, N);
+                            uint8_t &d = done[(size_t)o * nchunks + pc[ph]];
+                            if (d) return fail(cta, t, "output produced twice", y, z, 0);
+                            d = 1;
+                        }
+                    }
+                    if (ci >= 0) {
+                        if (mode != MODE_FULL) return fail(cta, t, "output point in a warp that skips the plane", y, z, 0);
+                        if (ce != ci) return fail(cta, t, "centre value", y, z, 0);
+                        for (int k = 1; k <= N; ++k) {
+                            if (sg[(N + y) * W + N + z + k] != arm(ci, 2, k)) return fail(cta, t, "z arm", y, z, k);
+                            if (sg[(N + y) * W + N + z - k] != arm(ci, 2, -k)) return fail(cta, t, "z arm", y, z, -k);
+                            if (sg[(N + y + k) * W + N + z] != arm(ci, 1, k)) return fail(cta, t, "y arm", y, z, k);
+                            if (sg[(N + y - k) * W + N + z] != arm(ci, 1, -k)) return fail(cta, t, "y arm", y, z, -k);
+                            if (hp[(ph + N - k) % N] != arm(ci, 0, -k)) return fail(cta, t, "backward x arm", y, z, -k);
+                        }
+                    }
+                    pp[ph] = ci;
+                    pc[ph] = chunk;
+                    hp[ph] = ce;
+                }
+        }
+        for (size_t q = 0; q < pend.size(); ++q)
+            if (pend[q] >= 0) return fail(cta, nsteps, "output still pending at the end of the CTA's steps", 0, 0, 0);
+    }
+    for (size_t q = 0; q < done.size(); ++q)
+        if (!done[q]) return "mesh point " + std::to_string(q / nchunks) + " slice " + std::to_string(q % nchunks) + " is never produced";
+    if (stats) {
+        stats[0] = nctas, stats[1] = h.nrec, stats[2] = npieces;
+        stats[3] = (int64_t)(h.cost_max * 1000), stats[4] = (int64_t)(h.cost_mean * 1000);
+        stats[5] = (int64_t)(h.items.size() * sizeof(int2) + h.recs.size());
+    }
+    return std::string();
 }

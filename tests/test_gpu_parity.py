@@ -44,7 +44,7 @@ def test_config0(kernel, ordering):
 
 
 # ---- config 1: benzene-shaped, nst=16, every block size 1..64 (padded) --------------------------
-@pytest.mark.parametrize("kernel", ["auto", "gather"])
+@pytest.mark.parametrize("kernel", ["auto", "gather", "sweep"])
 @pytest.mark.parametrize("B", [1, 2, 4, 8, 16, 32, 64])
 def test_config1_real(B, kernel):
     p = problem(1)
@@ -55,7 +55,7 @@ def test_config1_real(B, kernel):
     check(g, o, p.cond_denominator(psi, 4), f"config1 B={B}")
 
 
-@pytest.mark.parametrize("kernel", ["auto", "gather"])
+@pytest.mark.parametrize("kernel", ["auto", "gather", "sweep"])
 @pytest.mark.parametrize("B", [1, 2, 8, 32, 64])
 def test_config1_complex(B, kernel):
     p = problem(1)
@@ -77,6 +77,35 @@ def test_other_orders(n, kernel):
     g = _run(p, psi, n, 4, kernel)                                  # 5 orbitals in blocks of 4: 4 + 1 (padded)
     o = p.oracle_hpsi(psi, n)
     check(g, o, p.cond_denominator(psi, n), f"order {n}")
+
+
+@pytest.mark.parametrize("knob", [("sweep_tensor", 1), ("sweep_planes", 8), ("sweep_planes", 100), ("sweep_ctas", 7),
+                                  ("sweep_ctas", 1000)])
+def test_sweep_kernel_variants(knob):
+    """The plane-sweep kernel under its tuning knobs: 2-D tensor-map copies for 16 columns, thin and thick slabs,
+    few CTAs (long chains of work pieces through one CTA) and more CTAs than work."""
+    cfg = synthetic.config(1)
+    rs.rs_set_tuning(*knob)
+    try:
+        p = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=4)      # fresh mesh: tables built under the knob
+        psi = synthetic.orbitals(cfg.seed, 0, cfg.nst, p.np)
+        g = p.gpu_hpsi(psi, 4, 16, kernel=rs.RS_KERNEL_SWEEP)
+        assert rs.rs_kernel_name(p.mesh, 4, 16, kernel=rs.RS_KERNEL_SWEEP).startswith("sweep[")
+    finally:
+        rs.rs_set_tuning(knob[0], {"sweep_tensor": 0, "sweep_planes": 32, "sweep_ctas": 0}[knob[0]])
+    o = problem(1).oracle_hpsi(psi, 4)
+    check(g, o, problem(1).cond_denominator(psi, 4), f"sweep variant {knob}")
+
+
+def test_sweep_kernel_dirichlet_boxes():
+    """Non-periodic boxes through the plane-sweep kernel: sizes that are not multiples of the 16 x 16 tile."""
+    for box in [(24, 24, 24), (7, 9, 10), (1, 1, 37), (13, 1, 5), (40, 17, 33)]:
+        p = Problem(None, None, None, 0.25, max_n=4, box=box, periodic=False)
+        rng = np.random.default_rng(23)
+        psi = rng.standard_normal((16, p.np))
+        g = _run(p, psi, 4, 16, "sweep")
+        o = p.oracle_hpsi(psi, 4)
+        check(g, o, p.cond_denominator(psi, 4), f"sweep box {box}")
 
 
 def test_config1_order6_lex_ordering():

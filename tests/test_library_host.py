@@ -190,3 +190,30 @@ def test_no_cpu_fallback_without_a_device():
     with pytest.raises(rs.RsError) as e:
         rs.rs_hamiltonian_apply_states_host(m, 4, c, np.zeros(npts), np.zeros((4, npts)), np.zeros((4, npts)), 4)
     assert e.value.status == rs.RS_ERR_CUDA
+
+
+# ---- plane-sweep kernel's compact records: host replay against the plain neighbour table (reading S15) ----
+@pytest.mark.parametrize("cfg_i,nst,dtype,planes,nctas", [
+    (0, 16, rs.RS_REAL64, 32, 148), (0, 16, rs.RS_REAL64, 8, 3), (1, 16, rs.RS_REAL64, 32, 148),
+    (1, 32, rs.RS_REAL64, 32, 148), (1, 64, rs.RS_REAL64, 16, 132), (1, 8, rs.RS_COMPLEX128, 32, 148),
+    (1, 16, rs.RS_REAL64, 100, 1), (1, 16, rs.RS_REAL64, 12, 1000),
+])
+def test_sweep_records_expand_to_the_plain_table(cfg_i, nst, dtype, planes, nctas):
+    cfg = synthetic.config(cfg_i)
+    mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, 4)
+    st = rs.rs_sweep_selfcheck(mesh, 4, nst, dtype, planes, nctas)
+    assert st["nctas"] == nctas and st["records"] > 0 and st["cost_max"] >= st["cost_mean"] > 0
+
+
+def test_sweep_selfcheck_on_boxes_and_unsupported_calls():
+    for box in [(24, 24, 24), (7, 9, 10), (1, 1, 37), (40, 17, 33)]:
+        mesh = rs.rs_mesh_create_box(*box, 0.25, 4, False, rs.RS_ORDER_LEX)
+        rs.rs_sweep_selfcheck(mesh, 4, 16, rs.RS_REAL64, 32, 148)
+    mesh = rs.rs_mesh_create_box(8, 8, 8, 0.25, 4, True, rs.RS_ORDER_LEX)          # periodic: gather kernel only
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_sweep_selfcheck(mesh, 4, 16)
+    assert e.value.status == rs.RS_ERR_UNSUPPORTED
+    mesh = rs.rs_mesh_create_box(8, 8, 8, 0.25, 4, False, rs.RS_ORDER_LEX)
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_sweep_selfcheck(mesh, 4, 8)                                           # 8 real columns: gather kernel only
+    assert e.value.status == rs.RS_ERR_UNSUPPORTED
