@@ -160,6 +160,12 @@ rs_status rs_set_tuning(const char *name, int value);
 rs_status rs_sweep_selfcheck(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, int max_planes, int nctas,
                              int64_t *stats_host);
 
+/* Per-CTA figures of the plane-sweep kernel's last launch for (mesh, fd_order, nst, dtype), for calibrating
+ * the cost model that deals work to the persistent CTAs: out_host [max_ctas][5] = {clock ticks spent, steps,
+ * work pieces, modelled load x1000, full warp-steps}.  Synchronises the device.  Returns the number of
+ * CTAs written (0 if that kernel has not run).                                                           */
+int64_t rs_sweep_stats(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, int64_t *out_host, int64_t max_ctas);
+
 #ifdef __cplusplus
 }
 #endif

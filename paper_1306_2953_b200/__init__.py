@@ -36,7 +36,7 @@ EXPORTS = (
     "rs_mesh_spacing", "rs_mesh_nbricks", "rs_mesh_get_points", "rs_mesh_get_index_map", "rs_block_bytes",
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
     "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version", "rs_set_tuning",
-    "rs_sweep_selfcheck",
+    "rs_sweep_selfcheck", "rs_sweep_stats",
 )
 
 
@@ -81,6 +81,8 @@ def _load() -> C.CDLL:
     L.rs_kernel_table_bytes.restype = C.c_int64
     L.rs_version.restype = C.c_int
     L.rs_set_tuning.argtypes = [C.c_char_p, C.c_int]
+    L.rs_sweep_stats.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64), C.c_int64]
+    L.rs_sweep_stats.restype = C.c_int64
     L.rs_sweep_selfcheck.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]
     return L
 
@@ -167,6 +169,13 @@ def rs_version() -> int:
 
 def rs_set_tuning(name: str, value: int) -> None:
     _check(_lib.rs_set_tuning(name.encode(), value))
+
+
+def rs_sweep_stats(mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, max_ctas: int = 4096) -> np.ndarray:
+    """[nctas][5] int64: {clock ticks of the last launch, steps, pieces, modelled load x1000, full warp-steps} per CTA."""
+    out = np.zeros((max_ctas, 5), dtype=np.int64)
+    n = _lib.rs_sweep_stats(mesh.handle, fd_order, nst, dtype, out.ctypes.data_as(C.POINTER(C.c_int64)), max_ctas)
+    return out[:n]
 
 
 def rs_sweep_selfcheck(mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, max_planes: int = 32, nctas: int = 148) -> dict:

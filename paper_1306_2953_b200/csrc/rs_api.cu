@@ -165,6 +165,13 @@ extern "C" rs_status rs_set_tuning(const char *name, int value)
     return rs_fail(RS_ERR_INVALID_ARG, "rs_set_tuning: unknown knob");
 }
 
+int64_t rs_sweep_read_stats(const rs_mesh *cm, int n, int ncol, int64_t *out, int64_t max_ctas);
+extern "C" int64_t rs_sweep_stats(const rs_mesh *m, int n, int nst, rs_dtype dtype, int64_t *out_host, int64_t max_ctas)
+{
+    if (!m || !out_host || max_ctas < 1) return 0;
+    return rs_sweep_read_stats(m, n, nst * (dtype == RS_COMPLEX128 ? 2 : 1), out_host, max_ctas);
+}
+
 extern "C" rs_status rs_sweep_selfcheck(const rs_mesh *m, int n, int nst, rs_dtype dtype, int max_planes, int nctas,
                                         int64_t *stats_host)
 {

@@ -36,6 +36,7 @@ struct rs_sweep_host {
     std::vector<std::vector<rs_sweep_piece>> pieces; // per CTA, in execution order
     std::vector<unsigned char> recs;                 // [nrec][RS_SWEEP_REC_BYTES]
     int64_t nrec = 0;
+    std::vector<double> load;                        // modelled load per CTA
     double cost_max = 0.0, cost_mean = 0.0;          // modelled load of the busiest / average CTA
 };
 struct rs_sweep_tables {
@@ -43,6 +44,8 @@ struct rs_sweep_tables {
     int64_t nitems = 0, nrec = 0, bytes = 0;
     int2 *d_items = nullptr;
     unsigned char *d_recs = nullptr;
+    long long *d_cycles = nullptr;                   // per CTA: clock ticks of the last launch
+    std::vector<int64_t> host_stats;                 // per CTA: {steps, pieces, modelled load x 1000, full warp-steps}
 };
 
 struct rs_mesh {

@@ -50,7 +50,7 @@ constexpr int SW_SLOT_BYTES = SW_C * 8;  // 128
 constexpr int SW_STAGE_BYTES = SW_W * SW_W * SW_SLOT_BYTES;  // 73,728: uniform [24][24] slots; corners hold V, idx, header
 constexpr int SW_STAGES = 3;
 constexpr int SW_CONSUMERS = 256;        // 8 consumer warps
-constexpr int SW_THREADS = 384;          // + one producer warpgroup
+constexpr int SW_THREADS = 512;          // + two producer warpgroups (steps alternate between them)
 constexpr int SW_MAXRUN = RS_SWEEP_MAXRUN;
 constexpr int SW_TMEM_COLS = 512;        // allocated; used: 2 x (4 x 32 [centre ring] + 4 x 16 [offset ring])
 // packed per-plane record (rs_internal.h): runs | fill rows | header | indices of the tile's points
@@ -173,6 +173,21 @@ __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sy
 #undef W4
 #undef P4
 
+// predicated 8-byte store to base + 8 * off unless off is the invalid mark: no branch, one address instruction
+__device__ __forceinline__ void store_if_valid(double *base, uint32_t off, double v)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        ".reg .u64 q;\n"
+        "setp.ne.u32 p, %0, 0xffffffff;\n"
+        "mad.wide.u32 q, %0, 8, %1;\n"
+        "@p st.global.f64 [q], %2;\n"
+        "}\n" ::"r"(off),
+        "l"(base), "d"(v)
+        : "memory");
+}
+
 __device__ __forceinline__ double words2double(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
 
 // ---------------------------------------------------------------------------------------------
@@ -185,6 +200,7 @@ struct sweep_args {
     const double *psi;
     double *hpsi;
     uint32_t ncol;               // row pitch of the block in elements
+    long long *cycles;           // optional [gridDim.x]: clock64 ticks each CTA spent (calibration of the cost model)
 };
 struct sweep_maps {
     CUtensorMap box[SW_NBOX];    // psi as a [np+1][ncol] fp64 tensor, box {16, 1|2|4|8|16|24}
@@ -193,44 +209,73 @@ struct sweep_maps {
 // stage offsets of the small per-plane arrays kept in the unused corners of the [24][24] slot grid
 constexpr uint32_t SW_HDR_OFF = (uint32_t)((SW_W - SW_N) * SW_W) * SW_SLOT_BYTES;   // corner C: row 20, slot 0
 
-// ---- producer warpgroup (4 warps): stage plane after plane --------------------------------------------
-// Every warp takes a quarter of each job (copy runs, zero fill, V / index gather) and arrives once on the
-// stage's "full" barrier.  Records arrive through a ring of SW_RING slots, requested SW_LOOKAHEAD steps
-// ahead by thread 0: a warp working on step t proves that all warps finished step t - 3 (the consumers
-// released that stage), so the slot of record t - 3 = slot of record t + 3 may be overwritten.
+// Optional timeline of one CTA (development builds only, -DSW_TRACE): clock64 stamps per step after the per-CTA ticks.
+#ifndef SW_EXP
+#define SW_EXP 0   // development builds: bit 0 drops the FULL-mode stores, bit 1 the tensor-memory traffic, bit 2 the z/y loads
+#endif
+#ifdef SW_TRACE
+#define SW_STAMP(cond, t, k) do { if ((cond) && blockIdx.x == SW_TRACE && (t) < 256) a.cycles[gridDim.x + (t) * 8 + (k)] = clock64(); } while (0)
+#else
+#define SW_STAMP(cond, t, k) do { } while (0)
+#endif
+
+// ---- producer warps: two groups of 4 warps stage plane after plane, group g taking steps t = g (mod 2) ------
+// Inside a group every warp takes a quarter of each job (copy runs, zero fill, V / index gather) and arrives
+// once on the stage's "full" barrier.  Two groups because a step's chain of barrier waits, copy issues and
+// fences is latency-bound (~2000 clocks measured): two steps in flight double the rate.  Records arrive through
+// a ring of SW_RING slots; the group working on step t requests record t + SW_LOOKAHEAD: having passed the
+// "empty" wait of step t proves that the consumers, hence all producer warps, finished step t - 3, whose slot
+// is the one overwritten.
 template <bool TENSOR>
 __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_maps &maps, unsigned char *smem,
                                                uint32_t full0, uint32_t empty0, uint32_t rbar0, const unsigned char *recs,
                                                int nsteps, int ptid)
 {
     constexpr int N = SW_N;
-    const int lane = ptid & 31, pw = ptid >> 5;
+    const int group = ptid >> 7, gtid = ptid & 127, lane = ptid & 31, pw = gtid >> 5;
     unsigned char *const ring = smem + (size_t)SW_STAGES * SW_STAGE_BYTES;
     const uint32_t sbase = smem_u32(smem);
-    auto request_rec = [&](int r) {   // thread 0
+    auto request_rec = [&](int r) {   // one thread; preceded by a fence.proxy.async of that thread
         const uint32_t bar = rbar0 + 8u * (r % SW_RING);
-        fence_proxy_async();
         mbar_arrive_expect_tx(bar, SW_REC_BYTES);
         bulk_g2s(smem_u32(ring) + (uint32_t)(r % SW_RING) * SW_REC_BYTES, recs + (size_t)r * SW_REC_BYTES, SW_REC_BYTES, bar);
     };
     if (ptid == 0)
         for (int r = 0; r < SW_LOOKAHEAD && r < nsteps; ++r) request_rec(r);
-    // this thread's jobs: copy run `myrun` (lanes 0..15 of each warp), fill slots ptid + 128 k, tile points ptid and ptid + 128
+    // this thread's jobs: copy run `myrun` (lanes 0..15 of each warp), fill slots gtid + 128 k, tile points gtid and gtid + 128
     const int myrun = lane * 4 + pw;
-    int stage = 0, rs = 0;
-    uint32_t eparity = 1, rparity = 0;   // the first pass over the stages finds them free
-    for (int t = 0; t < nsteps; ++t) {
-        mbar_wait(empty0 + 8u * stage, eparity);
+    const int p0 = gtid, p1 = gtid + 128;
+    const uint32_t v_off0 = (uint32_t)(((p0 >> 6) * SW_W) * SW_SLOT_BYTES + (p0 & 63) * 8), v_off1 = v_off0 + 2 * SW_W * SW_SLOT_BYTES;
+    const uint32_t i_off0 = (uint32_t)(((p0 >> 6) * SW_W + SW_W - N) * SW_SLOT_BYTES + (p0 & 63) * 4), i_off1 = i_off0 + 2 * SW_W * SW_SLOT_BYTES;
+    int stage = group, rs = group;               // t mod SW_STAGES, t mod SW_RING
+    uint32_t eparity = 1, rparity = 0;           // the first pass over the stages finds them free
+    // V and the indices of a plane are fetched one step (of this group) ahead of their use, so that the
+    // global-load latency is not on the per-step path
+    int32_t ci0 = -1, ci1 = -1;
+    double vv0 = 0.0, vv1 = 0.0;
+    auto fetch_v = [&](int slot) {
+        const unsigned char *rp = ring + (size_t)slot * SW_REC_BYTES;
+        ci0 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p0 * 4);
+        ci1 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p1 * 4);
+        vv0 = ci0 >= 0 ? __ldg(a.vloc + ci0) : 0.0;
+        vv1 = ci1 >= 0 ? __ldg(a.vloc + ci1) : 0.0;
+    };
+    if (group < nsteps) {
         mbar_wait(rbar0 + 8u * rs, rparity);
-        const unsigned char *rp = ring + (size_t)rs * SW_REC_BYTES;
+        fetch_v(rs);
+    }
+    for (int t = group; t < nsteps; t += 2) {
+        SW_STAMP(gtid == 0, t, 0);
+        mbar_wait(empty0 + 8u * stage, eparity);
+        SW_STAMP(gtid == 0, t, 1);
+        fence_proxy_async();   // earlier generic accesses to this stage and to the record slot reused below (ordered before us by the barrier) before our async copies
+        if (gtid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
+        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 4);
+        const unsigned char *rp = ring + (size_t)rs * SW_REC_BYTES;   // record t: present, fetch_v waited for it
         const uint32_t sb = sbase + (uint32_t)stage * SW_STAGE_BYTES;
         unsigned char *const sg = smem + (size_t)stage * SW_STAGE_BYTES;
         const uint32_t bar = full0 + 8u * stage;
         const uint4 hdr = *reinterpret_cast<const uint4 *>(rp + SW_REC_HDR);   // {modes|flags, column offset, tx bytes 1-D, tx bytes 2-D}
-        if (ptid == 0) {
-            mbar_expect_tx(bar, TENSOR ? hdr.w : hdr.z);
-            *reinterpret_cast<uint2 *>(sg + SW_HDR_OFF) = make_uint2(hdr.x, hdr.y);
-        }
         // ---- copy runs --------------------------------------------------------------------------------
         if (lane < SW_MAXRUN / 4) {
             const uint2 r = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
@@ -248,46 +293,56 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
                 }
             }
         }
-        // ---- zero fill: bit s of the record's bitmap says that slot s of the [24][24] grid must be cleared ----
-#pragma unroll
-        for (int k = 0; k < (SW_W * SW_W + 127) / 128; ++k) {
-            const int sl = ptid + 128 * k;
-            if (sl < SW_W * SW_W) {
-                const uint32_t m = *reinterpret_cast<const uint32_t *>(rp + SW_REC_FILL + (sl >> 5) * 4);
-                if ((m >> (sl & 31)) & 1u) {
-                    float4 *d = reinterpret_cast<float4 *>(sg + (size_t)sl * SW_SLOT_BYTES);
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) d[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-                }
+        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 5);
+        // ---- zero fill: bit s of the record's bitmap says that slot s of the [24][24] grid must be cleared.  A warp
+        //      takes every 4th word of the bitmap; a quarter-warp clears one slot with 8 conflict-free 16-byte stores ----
+#pragma unroll 1
+        for (int wd = pw; wd < (SW_W * SW_W + 31) / 32; wd += 4) {
+            const uint32_t m = *reinterpret_cast<const uint32_t *>(rp + SW_REC_FILL + wd * 4);
+            if (m == 0) continue;
+#pragma unroll 1
+            for (int g4 = 0; g4 < 8; ++g4) {
+                if (((m >> (4 * g4)) & 15u) == 0) continue;
+                const int sl = wd * 32 + g4 * 4 + (lane >> 3);
+                if ((m >> (4 * g4 + (lane >> 3))) & 1u)
+                    *reinterpret_cast<float4 *>(sg + (size_t)sl * SW_SLOT_BYTES + (lane & 7) * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
         // ---- V and the mesh indices of the tile's own points (output planes only) ----------------------
         if (hdr.x & HDR_OUTPUT_PLANE) {
-            int32_t ci[2];
-            double vv[2];
-#pragma unroll
-            for (int q = 0; q < 2; ++q) ci[q] = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + (ptid + 128 * q) * 4);
-#pragma unroll
-            for (int q = 0; q < 2; ++q) vv[q] = ci[q] >= 0 ? __ldg(a.vloc + ci[q]) : 0.0;
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                const int p = ptid + 128 * q, ty = p >> 4, tz = p & 15;
-                *reinterpret_cast<double *>(sg + ((ty >> 2) * SW_W) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 8) = vv[q];
-                *reinterpret_cast<int32_t *>(sg + ((ty >> 2) * SW_W + SW_W - N) * SW_SLOT_BYTES + ((ty & 3) * 16 + tz) * 4) = ci[q];
-            }
+            *reinterpret_cast<double *>(sg + v_off0) = vv0;
+            *reinterpret_cast<double *>(sg + v_off1) = vv1;
+            *reinterpret_cast<int32_t *>(sg + i_off0) = ci0;
+            *reinterpret_cast<int32_t *>(sg + i_off1) = ci1;
         }
-        fence_proxy_async();
+        if (gtid == 0) *reinterpret_cast<uint2 *>(sg + SW_HDR_OFF) = make_uint2(hdr.x, hdr.y);
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar);
-        if (ptid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
-        if (++stage == SW_STAGES) {
-            stage = 0;
+        SW_STAMP(gtid == 0, t, 2);
+        // one arrival per warp; the group's first thread also announces the bytes of all the group's copies (the
+        // count may run negative until then: the phase cannot complete before this arrival)
+        if (lane == 0) {
+            if (pw == 0)
+                mbar_arrive_expect_tx(bar, TENSOR ? hdr.w : hdr.z);
+            else
+                mbar_arrive(bar);
+        }
+        SW_STAMP(gtid == 0, t, 3);
+        stage += 2;
+        if (stage >= SW_STAGES) {
+            stage -= SW_STAGES;
             eparity ^= 1u;
         }
-        if (++rs == SW_RING) {
-            rs = 0;
+        rs += 2;
+        if (rs >= SW_RING) {
+            rs -= SW_RING;
             rparity ^= 1u;
         }
+        if (t + 2 < nsteps) {   // this group's next step: its record was requested SW_LOOKAHEAD steps before it
+            mbar_wait(rbar0 + 8u * rs, rparity);
+            SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 6);
+            fetch_v(rs);
+        }
+        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 7);
     }
 }
 
@@ -336,7 +391,9 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             tm_wait_st();
             uint32_t io[16];
             tm_ld16(t_ix + PH * 16, io);
+            SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 4);
             mbar_wait(full0 + 8u * stage, parity);
+            SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 5);
             const unsigned char *sp = smem + (size_t)stage * SW_STAGE_BYTES;
             const uint2 hdr = *reinterpret_cast<const uint2 *>(sp + SW_HDR_OFF);   // {modes | flags, column offset}
             const int mode = (int)((hdr.x >> (2 * warp)) & 3u);
@@ -364,10 +421,13 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     uint32_t pw[32];   // centre values of planes t-1 .. t-4 of this patch row
-                    tm_ld32(t_in + j * 32, pw);
+                    if (!(SW_EXP & 2)) tm_ld32(t_in + j * 32, pw);
+                    else
+#pragma unroll
+                        for (int q = 0; q < 32; ++q) pw[q] = io[q & 15] + q;
                     double v[4 + 2 * N];
 #pragma unroll
-                    for (int tt = 0; tt < 4 + 2 * N; ++tt) v[tt] = pb[(j * SW_W + tt) * SW_C];
+                    for (int tt = 0; tt < 4 + 2 * N; ++tt) v[tt] = (SW_EXP & 4) ? (tt == N ? pb[(j * SW_W + tt) * SW_C] : (double)(tt + j) * w0x3) : pb[(j * SW_W + tt) * SW_C];
                     const double2 va = *reinterpret_cast<const double2 *>(sp + vrow + j * 128);
                     const double2 vb = *reinterpret_cast<const double2 *>(sp + vrow + j * 128 + 16);
                     const double vv[4] = {va.x, va.y, vb.x, vb.y};
@@ -379,7 +439,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
 #pragma unroll
                         for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
                         const double out = fma(w.w[N], ce, acc[PH][j][i]);
-                        if (io[4 * j + i] != 0xffffffffu) hp[io[4 * j + i]] = out;
+                        if (!(SW_EXP & 1)) store_if_valid(hp, io[4 * j + i], out);
                         s[i] = (w0x3 + vv[i]) * ce;
 #pragma unroll
                         for (int k = 1; k <= N; ++k) {
@@ -388,7 +448,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                         }
                     }
                     // backward half of the x arm from tensor memory, then park this row's centre values
-                    tm_wait_ld32(pw);
+                    if (!(SW_EXP & 2)) tm_wait_ld32(pw);
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
 #pragma unroll
@@ -404,7 +464,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                         cw[2 * i] = (uint32_t)__double2loint(ctr[j][i]);
                         cw[2 * i + 1] = (uint32_t)__double2hiint(ctr[j][i]);
                     }
-                    tm_st8(t_in + j * 32 + PH * 8, cw);
+                    if (!(SW_EXP & 2)) tm_st8(t_in + j * 32 + PH * 8, cw);
                 }
                 // y arms: rows 4py-4 .. 4py+7 of the patch's 4 z columns
 #pragma unroll
@@ -412,7 +472,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                     double u[4 + 2 * N];
 #pragma unroll
                     for (int tt = 0; tt < 4 + 2 * N; ++tt)
-                        u[tt] = (tt >= N && tt < N + 4) ? ctr[tt - N][i] : pb[((tt - N) * SW_W + N + i) * SW_C];
+                        u[tt] = (tt >= N && tt < N + 4) ? ctr[tt - N][i] : ((SW_EXP & 4) ? (double)(tt + i) * w0x3 : pb[((tt - N) * SW_W + N + i) * SW_C]);
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
 #pragma unroll
@@ -432,7 +492,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
 #pragma unroll
                         for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
                         const double out = fma(w.w[N], ce, acc[PH][j][i]);
-                        if (io[4 * j + i] != 0xffffffffu) hp[io[4 * j + i]] = out;
+                        store_if_valid(hp, io[4 * j + i], out);
                         acc[PH][j][i] = 0.0;
                         cw[2 * i] = (uint32_t)__double2loint(ce);
                         cw[2 * i + 1] = (uint32_t)__double2hiint(ce);
@@ -448,7 +508,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                 for (int j = 0; j < 4; ++j) {
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
-                        if (io[4 * j + i] != 0xffffffffu) hp[io[4 * j + i]] = acc[PH][j][i];
+                        store_if_valid(hp, io[4 * j + i], acc[PH][j][i]);
                         acc[PH][j][i] = 0.0;
                     }
                     tm_st8(t_in + j * 32 + PH * 8, cw);
@@ -456,6 +516,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             }
             // this warp has read everything it needs from the stage
             __syncwarp();
+            SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 6);
             if (lane == 0) mbar_arrive(empty0 + 8u * stage);
             if (++stage == SW_STAGES) {
                 stage = 0;
@@ -479,11 +540,12 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     const int tid = threadIdx.x, warp = tid >> 5;
     const int2 item = a.items[blockIdx.x];
     const int nsteps = item.y;
+    const long long clock0 = clock64();
 
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < SW_STAGES; ++s) {
-            mbar_init(smem_u32(&full_bar[s]), (SW_THREADS - SW_CONSUMERS) / 32);
+            mbar_init(smem_u32(&full_bar[s]), 4);   // the 4 warps of the producer group that stages the step
             mbar_init(smem_u32(&empty_bar[s]), SW_CONSUMERS / 32);
         }
 #pragma unroll
@@ -500,16 +562,17 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
 
-    // register re-split: 384 x 168 at launch = 128 x 40 (producer group) + 256 x 232 (consumers); the pool that
+    // register re-split: 512 x 128 at launch = 256 x 24 (producers) + 256 x 232 (consumers); the pool that
     // setmaxnreg.inc draws from holds only what setmaxnreg.dec released, so the two must balance exactly
     if (tid >= SW_CONSUMERS) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 32;\n");
         sweep_producer<TENSOR>(a, maps, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), smem_u32(&rec_bar[0]),
                                a.recs + (size_t)item.x * SW_REC_BYTES, nsteps, tid - SW_CONSUMERS);
     } else {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;\n");
         sweep_consumer(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, tid);
         named_bar_sync(1, SW_CONSUMERS);
+        if (tid == 0 && a.cycles) a.cycles[blockIdx.x] = clock64() - clock0;
         if (warp == 0)
             asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base_s), "n"(SW_TMEM_COLS) : "memory");
     }
@@ -529,10 +592,13 @@ void rs_sweep_set_nctas(int v) { g_nctas = v < 0 ? 0 : v; }
 
 namespace {
 
-// modelled cost of one consumer-warp step by mode (relative to a full step), and of a whole step:
-// warps w and w + 4 share a scheduler, the busiest scheduler paces the step
-constexpr double COST_MODE[3] = {0.04, 0.15, 1.0};
-constexpr double COST_STEP_FIXED = 0.05;
+// modelled cost of a step, in units of a step whose 8 warps are all in full mode.  Least-squares fit of the per-CTA
+// clock counts of the kernel itself (rs_sweep_stats; config 2, B = 16 on B200, rms error 3 %):
+//   clocks = 1976 steps + 124 full warp-steps + 2484 pieces   (a full step: 1976 + 8 x 124 = 2968 clocks)
+// i.e. two thirds of a step's time does not depend on how many warps compute: it is the latency of the
+// release -> stage -> copy -> consume chain through the 3 stage buffers.
+constexpr double COST_STEP_FIXED = 0.666, COST_FULL_WARP = 0.042, COST_CENTRE_WARP = 0.006, COST_PIECE = 0.84;
+constexpr double COST_EMPTY_STEP = COST_STEP_FIXED;
 
 struct tile_geometry {
     const rs_mesh *m;
@@ -558,12 +624,12 @@ struct tile_geometry {
 
 double step_cost(uint32_t modes)
 {
-    double worst = 0.0;
-    for (int q = 0; q < 4; ++q) {
-        const double c = COST_MODE[(modes >> (2 * q)) & 3u] + COST_MODE[(modes >> (2 * (q + 4))) & 3u];
-        worst = std::max(worst, c);
+    double c = COST_STEP_FIXED;
+    for (int q = 0; q < 8; ++q) {
+        const uint32_t md = (modes >> (2 * q)) & 3u;
+        c += md == MODE_FULL ? COST_FULL_WARP : md == MODE_CENTRE ? COST_CENTRE_WARP : 0.0;
     }
-    return COST_STEP_FIXED + 0.5 * worst;
+    return c;
 }
 
 }  // namespace
@@ -587,19 +653,19 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                     ccost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(g.warp_modes(iy, iz, x, MODE_CENTRE));
                 }
             }
-    auto halo_cost = [&](int iy, int iz, int xa, int xb) {   // the 2 N centre-only steps around [xa, xb)
-        double c = 0.0;
+    auto halo_cost = [&](int iy, int iz, int xa, int xb) {   // the 2 N centre-only steps around [xa, xb) + the piece's own overhead
+        double c = COST_PIECE;
         const double *cc = &ccost[((size_t)iy * g.ntz + iz) * nx];
         for (int k = 1; k <= N; ++k) {
-            c += (xa - k >= 0 && cc[xa - k] > 0.0) ? cc[xa - k] : COST_STEP_FIXED + 0.5 * 2 * COST_MODE[MODE_EMPTY];
-            c += (xb + k - 1 < nx && cc[xb + k - 1] > 0.0) ? cc[xb + k - 1] : COST_STEP_FIXED + 0.5 * 2 * COST_MODE[MODE_EMPTY];
+            c += (xa - k >= 0 && cc[xa - k] > 0.0) ? cc[xa - k] : COST_EMPTY_STEP;
+            c += (xb + k - 1 < nx && cc[xb + k - 1] > 0.0) ? cc[xb + k - 1] : COST_EMPTY_STEP;
         }
         return c;
     };
     auto range_cost = [&](int iy, int iz, int xa, int xb) {
         double c = 0.0;
         const double *fc = &fcost[((size_t)iy * g.ntz + iz) * nx];
-        for (int x = xa; x < xb; ++x) c += fc[x] > 0.0 ? fc[x] : COST_STEP_FIXED + 0.5 * 2 * COST_MODE[MODE_EMPTY];
+        for (int x = xa; x < xb; ++x) c += fc[x] > 0.0 ? fc[x] : COST_EMPTY_STEP;
         return c;
     };
 
@@ -658,7 +724,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                 double c = halo_cost(it.iy, it.iz, it.xa, it.xb);
                 const double *fc = &fcost[((size_t)it.iy * g.ntz + it.iz) * nx];
                 while (xsplit < it.xb - MIN_SPLIT) {
-                    const double cx = fc[xsplit] > 0.0 ? fc[xsplit] : COST_STEP_FIXED + COST_MODE[MODE_EMPTY];
+                    const double cx = fc[xsplit] > 0.0 ? fc[xsplit] : COST_EMPTY_STEP;
                     if (load[cta] + c + cx > finish) break;
                     c += cx;
                     ++xsplit;
@@ -688,6 +754,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
             lo = mid;
     }
     deal(hi, out.pieces);
+    out.load = load;
     for (double l : load) {
         out.cost_max = std::max(out.cost_max, l);
         out.cost_mean += l / nctas;
@@ -788,6 +855,16 @@ static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables *
             };
             RS_CUDA_TRY(up((void **)&tb.d_items, h.items.data(), h.items.size() * sizeof(int2)));
             RS_CUDA_TRY(up((void **)&tb.d_recs, h.recs.data(), h.recs.size()));
+            RS_CUDA_TRY(cudaMalloc((void **)&tb.d_cycles, (h.items.size() + 2048) * sizeof(long long)));
+            RS_CUDA_TRY(cudaMemset(tb.d_cycles, 0, (h.items.size() + 2048) * sizeof(long long)));
+            for (size_t c = 0; c < h.items.size(); ++c) {
+                int64_t nfull = 0;
+                for (int t = 0; t < h.items[c].y; ++t) {
+                    const uint32_t hd = *reinterpret_cast<const uint32_t *>(h.recs.data() + (size_t)(h.items[c].x + t) * SW_REC_BYTES + SW_REC_HDR);
+                    for (int wq = 0; wq < 8; ++wq) nfull += ((hd >> (2 * wq)) & 3u) == MODE_FULL;
+                }
+                tb.host_stats.insert(tb.host_stats.end(), {(int64_t)h.items[c].y, (int64_t)h.pieces[c].size(), (int64_t)(h.load[c] * 1000), nfull});
+            }
             RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
             RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
         }
@@ -837,6 +914,7 @@ rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const d
     sweep_args a;
     a.items = tb->d_items, a.recs = tb->d_recs;
     a.vloc = vloc, a.psi = psi, a.hpsi = hpsi, a.ncol = (uint32_t)ncol;
+    a.cycles = tb->d_cycles;
     sweep_maps maps;
     const bool tensor = ncol != SW_C || g_force_tensor;
     if (tensor) {
@@ -882,7 +960,7 @@ void rs_sweep_free(rs_mesh *m)
 {
     for (auto &kv : m->sweep) {
         rs_sweep_tables &t = kv.second;
-        cudaFree(t.d_items), cudaFree(t.d_recs);
+        cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles);
     }
     m->sweep.clear();
 }
@@ -990,4 +1068,26 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
         stats[5] = (int64_t)(h.items.size() * sizeof(int2) + h.recs.size());
     }
     return std::string();
+}
+
+// per-CTA {clock ticks of the last launch, steps, pieces, modelled load x 1000, full warp-steps}; returns the number of CTAs
+int64_t rs_sweep_read_stats(const rs_mesh *cm, int n, int ncol, int64_t *out, int64_t max_ctas)
+{
+    rs_mesh *m = const_cast<rs_mesh *>(cm);
+    auto f = m->sweep.find(std::make_pair(n, ncol));
+    if (f == m->sweep.end() || !f->second.ok) return 0;
+    const rs_sweep_tables &t = f->second;
+    const int64_t nc = std::min<int64_t>(t.nitems, max_ctas);
+    std::vector<long long> cyc(t.nitems + 2048);
+    if (cudaMemcpy(cyc.data(), t.d_cycles, cyc.size() * sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess) return 0;
+#ifdef SW_TRACE
+    if (max_ctas >= t.nitems + 410) {   // development builds: the timeline follows the per-CTA rows
+        for (int64_t q = 0; q < 2048; ++q) out[5 * t.nitems + q] = cyc[t.nitems + q];
+    }
+#endif
+    for (int64_t c = 0; c < nc; ++c) {
+        out[5 * c] = cyc[c];
+        for (int k = 0; k < 4; ++k) out[5 * c + 1 + k] = t.host_stats[4 * c + k];
+    }
+    return nc;
 }
