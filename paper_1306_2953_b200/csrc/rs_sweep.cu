@@ -229,7 +229,7 @@ constexpr uint32_t SW_HDR_OFF = (uint32_t)((SW_W - SW_N) * SW_W) * SW_SLOT_BYTES
 template <bool TENSOR>
 __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_maps &maps, unsigned char *smem,
                                                uint32_t full0, uint32_t empty0, uint32_t rbar0, const unsigned char *recs,
-                                               int nsteps, int ptid)
+                                               int nsteps, int ptid, double w0x3)
 {
     constexpr int N = SW_N;
     const int group = ptid >> 7, gtid = ptid & 127, lane = ptid & 31, pw = gtid >> 5;
@@ -257,8 +257,8 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         const unsigned char *rp = ring + (size_t)slot * SW_REC_BYTES;
         ci0 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p0 * 4);
         ci1 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p1 * 4);
-        vv0 = ci0 >= 0 ? __ldg(a.vloc + ci0) : 0.0;
-        vv1 = ci1 >= 0 ? __ldg(a.vloc + ci1) : 0.0;
+        vv0 = ci0 >= 0 ? __ldg(a.vloc + ci0) + w0x3 : 0.0;   // 3 w_0 + V: the whole diagonal coefficient
+        vv1 = ci1 >= 0 ? __ldg(a.vloc + ci1) + w0x3 : 0.0;
     };
     if (group < nsteps) {
         mbar_wait(rbar0 + 8u * rs, rparity);
@@ -266,33 +266,34 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
     }
     for (int t = group; t < nsteps; t += 2) {
         SW_STAMP(gtid == 0, t, 0);
-        mbar_wait(empty0 + 8u * stage, eparity);
-        SW_STAMP(gtid == 0, t, 1);
-        fence_proxy_async();   // earlier generic accesses to this stage and to the record slot reused below (ordered before us by the barrier) before our async copies
-        if (gtid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
-        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 4);
-        const unsigned char *rp = ring + (size_t)rs * SW_REC_BYTES;   // record t: present, fetch_v waited for it
+        // everything the copies need is read from the record (present: fetch_v waited for it) BEFORE the wait for
+        // the stage, so that the copies leave right after the consumers release it
+        const unsigned char *rp = ring + (size_t)rs * SW_REC_BYTES;
         const uint32_t sb = sbase + (uint32_t)stage * SW_STAGE_BYTES;
         unsigned char *const sg = smem + (size_t)stage * SW_STAGE_BYTES;
         const uint32_t bar = full0 + 8u * stage;
         const uint4 hdr = *reinterpret_cast<const uint4 *>(rp + SW_REC_HDR);   // {modes|flags, column offset, tx bytes 1-D, tx bytes 2-D}
+        uint2 run = make_uint2(0u, 0u);
+        if (lane < SW_MAXRUN / 4) run = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
+        const uint32_t len = run.y >> 16, slot = run.y & 0xffffu;
+        mbar_wait(empty0 + 8u * stage, eparity);
+        SW_STAMP(gtid == 0, t, 1);
+        fence_proxy_async();   // earlier generic accesses to this stage and to the record slot reused below (ordered before us by the barrier) before our async copies
         // ---- copy runs --------------------------------------------------------------------------------
-        if (lane < SW_MAXRUN / 4) {
-            const uint2 r = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
-            const uint32_t len = r.y >> 16, slot = r.y & 0xffffu;
-            if (len) {
-                if constexpr (!TENSOR) {
-                    bulk_g2s(sb + slot * SW_SLOT_BYTES, a.psi + (size_t)r.x * SW_C, len * SW_SLOT_BYTES, bar);
-                } else {
-                    // largest box height (1, 2, 4, 8, 16 or 24) not above len; a second, overlapping box covers the rest
-                    const int lg = len >= 24 ? 5 : 31 - __clz((int)len);
-                    const uint32_t p = len >= 24 ? 24u : 1u << lg;
-                    tensor_g2s(sb + slot * SW_SLOT_BYTES, &maps.box[lg], (int)hdr.y, (int)r.x, bar);
-                    if (p < len)
-                        tensor_g2s(sb + (slot + len - p) * SW_SLOT_BYTES, &maps.box[lg], (int)hdr.y, (int)(r.x + len - p), bar);
-                }
+        if (len) {
+            if constexpr (!TENSOR) {
+                bulk_g2s(sb + slot * SW_SLOT_BYTES, a.psi + (size_t)run.x * SW_C, len * SW_SLOT_BYTES, bar);
+            } else {
+                // largest box height (1, 2, 4, 8, 16 or 24) not above len; a second, overlapping box covers the rest
+                const int lg = len >= 24 ? 5 : 31 - __clz((int)len);
+                const uint32_t p = len >= 24 ? 24u : 1u << lg;
+                tensor_g2s(sb + slot * SW_SLOT_BYTES, &maps.box[lg], (int)hdr.y, (int)run.x, bar);
+                if (p < len)
+                    tensor_g2s(sb + (slot + len - p) * SW_SLOT_BYTES, &maps.box[lg], (int)hdr.y, (int)(run.x + len - p), bar);
             }
         }
+        if (gtid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
+        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 4);
         SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 5);
         // ---- zero fill: bit s of the record's bitmap says that slot s of the [24][24] grid must be cleared.  A warp
         //      takes every 4th word of the bitmap; a quarter-warp clears one slot with 8 conflict-free 16-byte stores ----
@@ -440,7 +441,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                         for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
                         const double out = fma(w.w[N], ce, acc[PH][j][i]);
                         if (!(SW_EXP & 1)) store_if_valid(hp, io[4 * j + i], out);
-                        s[i] = (w0x3 + vv[i]) * ce;
+                        s[i] = vv[i] * ce;   // vv = 3 w_0 + V, formed by the producer
 #pragma unroll
                         for (int k = 1; k <= N; ++k) {
                             s[i] = fma(w.w[k], v[N + i + k], s[i]);
@@ -567,7 +568,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     if (tid >= SW_CONSUMERS) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 32;\n");
         sweep_producer<TENSOR>(a, maps, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), smem_u32(&rec_bar[0]),
-                               a.recs + (size_t)item.x * SW_REC_BYTES, nsteps, tid - SW_CONSUMERS);
+                               a.recs + (size_t)item.x * SW_REC_BYTES, nsteps, tid - SW_CONSUMERS, 3.0 * w.w[0]);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;\n");
         sweep_consumer(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, tid);
