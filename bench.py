@@ -291,11 +291,13 @@ def main() -> None:
                 "peak_source": peak_src, "traffic": None, "algorithmic_bytes_per_launch": alg_bytes,
                 "apply_ms_per_launch": apply_ms, "apply_share_of_step": apply_ms * nblocks / ms_step,
                 "apply_gflops": B * npts * flops_per_output(n) * (4 if is_c else 1) / (apply_ms * 1e-3) / 1e9}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(traffic_file):      # dram bytes per launch from the committed ncu --set full capture
-        tr = json.load(open(traffic_file)).get(f"config{cfg.index}_B{B}_n{n}_{kname}")
-        if tr:
-            roofline["traffic"] = tr
+        import csv
+        key = f"config{cfg.index}_B{B}_n{n}_{kname}"
+        for row in csv.DictReader(open(traffic_file)):
+            if row["key"] == key:
+                roofline["traffic"] = int(row["dram_bytes_per_launch"])
 
     # ---- block-size sweep of the apply kernel alone (the metric is "vs orbital block size") -------
     sweep = None

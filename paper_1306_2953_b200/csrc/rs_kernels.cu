@@ -3,11 +3,11 @@
 
 // ---------------------------------------------------------------------------------------------
 // pack / unpack: tiled transpose through shared memory (Fig. 4 :107).
-// Tile = TP points x B orbitals.  Reads of `states` are contiguous along the point index, writes of
-// `block` are contiguous along (point, orbital); the smem tile is [B][TP+1] (padded: conflict-free).
+// Reads of `states` are contiguous along the point index, writes of `block` are contiguous along
+// (point, orbital); the smem tile is [B][tp+1] (padded: conflict-free).
+// Tile = tp points x B orbitals with tp * B = 2048 elements (tp a power of two in 32..256): 8 independent
+// loads in flight per thread, reads of 256-byte runs of one orbital, writes of whole 128-byte block rows.
 // ---------------------------------------------------------------------------------------------
-constexpr int TP = 32;
-
 template <typename T>
 __device__ __forceinline__ T zero_of();
 template <>
@@ -23,41 +23,45 @@ __device__ __forceinline__ double2 zero_of<double2>()
 
 template <typename T>
 __global__ void __launch_bounds__(256) pack_kernel(const T *__restrict__ states, int64_t ld, int ist0, int nst_in, int B,
-                                                   int logB, int64_t np, T *__restrict__ block)
+                                                   int logB, int logTP, int64_t np, T *__restrict__ block)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *tile = reinterpret_cast<T *>(smem_raw);
-    const int64_t ip0 = (int64_t)blockIdx.x * TP;
-    const int total = B * TP;
-    for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
-        const int j = idx / TP, p = idx % TP;
+    const int tp = 1 << logTP, total = B << logTP;
+    const int64_t ip0 = (int64_t)blockIdx.x << logTP;
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < total; idx += 256) {
+        const int j = idx >> logTP, p = idx & (tp - 1);
         T v = zero_of<T>();
-        if (j < nst_in && ip0 + p < np) v = states[(int64_t)(ist0 + j) * ld + ip0 + p];
-        tile[j * (TP + 1) + p] = v;
+        if (j < nst_in && ip0 + p < np) v = __ldg(states + (int64_t)(ist0 + j) * ld + ip0 + p);
+        tile[j * (tp + 1) + p] = v;
     }
     __syncthreads();
-    for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < total; idx += 256) {
         const int p = idx >> logB, j = idx & (B - 1);
-        if (ip0 + p <= np) block[((ip0 + p) << logB) + j] = tile[j * (TP + 1) + p];  // row np: zero slot
+        if (ip0 + p <= np) block[((ip0 + p) << logB) + j] = tile[j * (tp + 1) + p];  // row np: zero slot
     }
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) unpack_kernel(const T *__restrict__ block, int B, int logB, int nst_in, int64_t np,
-                                                     T *__restrict__ states, int64_t ld, int ist0)
+__global__ void __launch_bounds__(256) unpack_kernel(const T *__restrict__ block, int B, int logB, int logTP, int nst_in,
+                                                     int64_t np, T *__restrict__ states, int64_t ld, int ist0)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *tile = reinterpret_cast<T *>(smem_raw);
-    const int64_t ip0 = (int64_t)blockIdx.x * TP;
-    const int total = B * TP;
-    for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+    const int tp = 1 << logTP, total = B << logTP;
+    const int64_t ip0 = (int64_t)blockIdx.x << logTP;
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < total; idx += 256) {
         const int p = idx >> logB, j = idx & (B - 1);
-        if (ip0 + p < np) tile[j * (TP + 1) + p] = block[((ip0 + p) << logB) + j];
+        if (ip0 + p < np) tile[j * (tp + 1) + p] = __ldg(block + ((ip0 + p) << logB) + j);
     }
     __syncthreads();
-    for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
-        const int j = idx / TP, p = idx % TP;
-        if (j < nst_in && ip0 + p < np) states[(int64_t)(ist0 + j) * ld + ip0 + p] = tile[j * (TP + 1) + p];
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < total; idx += 256) {
+        const int j = idx >> logTP, p = idx & (tp - 1);
+        if (j < nst_in && ip0 + p < np) states[(int64_t)(ist0 + j) * ld + ip0 + p] = tile[j * (tp + 1) + p];
     }
 }
 
@@ -68,17 +72,25 @@ static int ilog2(int v)
     return l;
 }
 
+static int tile_log2(int B)   // points per tile: 2048 / B clamped to 32 .. 256
+{
+    int tp = 2048 / B;
+    tp = tp < 32 ? 32 : tp > 256 ? 256 : tp;
+    return ilog2(tp);
+}
+
 rs_status rs_launch_pack(const rs_mesh *m, const void *states, int64_t ld, int ist0, int nst_in, int B, void *block,
                          int lanes, cudaStream_t st)
 {
-    const unsigned grid = (unsigned)((m->np + 1 + TP - 1) / TP);
+    const int ltp = tile_log2(B), tp = 1 << ltp;
+    const unsigned grid = (unsigned)((m->np + 1 + tp - 1) / tp);
     const size_t esz = lanes == 2 ? 16 : 8;
-    const size_t smem = (size_t)B * (TP + 1) * esz;
+    const size_t smem = (size_t)B * (tp + 1) * esz;
     if (lanes == 2)
-        pack_kernel<double2><<<grid, 256, smem, st>>>((const double2 *)states, ld, ist0, nst_in, B, ilog2(B), m->np,
+        pack_kernel<double2><<<grid, 256, smem, st>>>((const double2 *)states, ld, ist0, nst_in, B, ilog2(B), ltp, m->np,
                                                       (double2 *)block);
     else
-        pack_kernel<double><<<grid, 256, smem, st>>>((const double *)states, ld, ist0, nst_in, B, ilog2(B), m->np,
+        pack_kernel<double><<<grid, 256, smem, st>>>((const double *)states, ld, ist0, nst_in, B, ilog2(B), ltp, m->np,
                                                      (double *)block);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
@@ -87,14 +99,15 @@ rs_status rs_launch_pack(const rs_mesh *m, const void *states, int64_t ld, int i
 rs_status rs_launch_unpack(const rs_mesh *m, const void *block, int B, int nst_in, void *states, int64_t ld, int ist0,
                            int lanes, cudaStream_t st)
 {
-    const unsigned grid = (unsigned)((m->np + TP - 1) / TP);
+    const int ltp = tile_log2(B), tp = 1 << ltp;
+    const unsigned grid = (unsigned)((m->np + tp - 1) / tp);
     const size_t esz = lanes == 2 ? 16 : 8;
-    const size_t smem = (size_t)B * (TP + 1) * esz;
+    const size_t smem = (size_t)B * (tp + 1) * esz;
     if (lanes == 2)
-        unpack_kernel<double2><<<grid, 256, smem, st>>>((const double2 *)block, B, ilog2(B), nst_in, m->np,
+        unpack_kernel<double2><<<grid, 256, smem, st>>>((const double2 *)block, B, ilog2(B), ltp, nst_in, m->np,
                                                         (double2 *)states, ld, ist0);
     else
-        unpack_kernel<double><<<grid, 256, smem, st>>>((const double *)block, B, ilog2(B), nst_in, m->np,
+        unpack_kernel<double><<<grid, 256, smem, st>>>((const double *)block, B, ilog2(B), ltp, nst_in, m->np,
                                                        (double *)states, ld, ist0);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;

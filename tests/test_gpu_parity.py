@@ -238,3 +238,40 @@ def test_kernel_choice_is_reported():
     name = rs.rs_kernel_name(p.mesh, 4, 16)
     assert name == "gather" or name.startswith("sweep[")
     assert rs.rs_kernel_table_bytes(p.mesh, 4, 16, kernel=rs.RS_KERNEL_GATHER) == p.np * 24 * 4
+
+
+# ---- full-size configs (BASELINE.json configs[2..4]) in the launch configuration bench.py times -----------
+# One block of orbitals through pack -> apply -> unpack on the full mesh, every output compared with the
+# oracle (the oracle does a whole orbital of these meshes in a fraction of a second per core).
+@pytest.mark.parametrize("B", [16, 32, 64])
+def test_config2_full_mesh_block(B):
+    p = problem(2)
+    cfg = p.cfg
+    nst = B + 3 if B == 16 else B                       # B = 16: a second, ragged block as well
+    psi = synthetic.orbitals(cfg.seed, 0, nst, p.np)
+    g = _run(p, psi, 4, B, "auto")
+    assert rs.rs_kernel_name(p.mesh, 4, B).startswith("sweep[")
+    o = p.oracle_hpsi(psi, 4, nthreads=16)
+    check(g, o, p.cond_denominator(psi, 4), f"config2 B={B}")
+
+
+@pytest.mark.parametrize("B", [8, 32])
+def test_config3_complex_full_mesh_block(B):
+    p = problem(2)                                       # config 3 = config 2's mesh and potential, complex orbitals
+    cfg = synthetic.config(3)
+    psi = synthetic.orbitals(cfg.seed, 0, B, p.np, is_complex=True)
+    g = _run(p, psi, 4, B, "auto")
+    assert rs.rs_kernel_name(p.mesh, 4, B, rs.RS_COMPLEX128).startswith("sweep[")
+    o = p.oracle_hpsi(psi, 4, nthreads=16)
+    check(g, o, p.cond_denominator(psi, 4), f"config3 complex B={B}")
+
+
+@pytest.mark.parametrize("n,B", [(4, 16), (4, 64), (6, 16)])
+def test_config4_full_mesh_block(n, B):
+    p = problem(4)                                       # 500 centres, 3.8 M points; orders 4 and 6
+    cfg = p.cfg
+    nst = min(B, 16)                                     # 16 orbitals (padded block for B = 64): the oracle's share stays small
+    psi = synthetic.orbitals(cfg.seed, 0, nst, p.np)
+    g = _run(p, psi, n, B, "auto")
+    o = p.oracle_hpsi(psi, n, nthreads=16)
+    check(g, o, p.cond_denominator(psi, n), f"config4 n={n} B={B}")
