@@ -1,5 +1,6 @@
 // C-ABI entry points: argument checks, weight formation, kernel dispatch, host-buffer sweep.
 #include <cstring>
+#include <vector>
 
 #include "rs_internal.h"
 
@@ -101,43 +102,67 @@ extern "C" rs_status rs_hamiltonian_apply_states_host(const rs_mesh *m, int n, c
     if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
     const size_t esz = dtype == RS_COMPLEX128 ? 16 : 8;
     const size_t sbytes = (size_t)nst_total * ld * esz, bbytes = rs_block_bytes(m, B, dtype);
-    void *d_states = nullptr, *d_out = nullptr, *d_psi = nullptr, *d_hpsi = nullptr;
+    // Three streams: upload of block k + 1, compute of block k and download of block k - 1 overlap (PCIe is full duplex);
+    // two pairs of block buffers so that compute never waits for its own previous unpack to drain.
+    void *d_states = nullptr, *d_out = nullptr, *d_psi[2] = {nullptr, nullptr}, *d_hpsi[2] = {nullptr, nullptr};
     double *d_v = nullptr;
-    cudaStream_t st = nullptr;
+    cudaStream_t s_in = nullptr, s_cmp = nullptr, s_out = nullptr;
+    const int nblocks = (nst_total + B - 1) / B;
+    std::vector<cudaEvent_t> ev_in(nblocks, nullptr), ev_cmp(nblocks, nullptr);
     rs_status rc = RS_OK;
     auto cleanup = [&]() {
-        cudaFree(d_states), cudaFree(d_out), cudaFree(d_psi), cudaFree(d_hpsi), cudaFree(d_v);
-        if (st) cudaStreamDestroy(st);
+        cudaFree(d_states), cudaFree(d_out), cudaFree(d_psi[0]), cudaFree(d_psi[1]), cudaFree(d_hpsi[0]), cudaFree(d_hpsi[1]), cudaFree(d_v);
+        for (cudaEvent_t e : ev_in)
+            if (e) cudaEventDestroy(e);
+        for (cudaEvent_t e : ev_cmp)
+            if (e) cudaEventDestroy(e);
+        if (s_in) cudaStreamDestroy(s_in);
+        if (s_cmp) cudaStreamDestroy(s_cmp);
+        if (s_out) cudaStreamDestroy(s_out);
     };
 #define TRY_OR_CLEAN(call)                                                                     \
     do {                                                                                       \
         cudaError_t _e = (call);                                                               \
         if (_e != cudaSuccess) {                                                               \
+            cudaDeviceSynchronize();                                                           \
             cleanup();                                                                         \
             return rs_fail(RS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e));   \
         }                                                                                      \
     } while (0)
-    TRY_OR_CLEAN(cudaStreamCreate(&st));
+    TRY_OR_CLEAN(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+    TRY_OR_CLEAN(cudaStreamCreateWithFlags(&s_cmp, cudaStreamNonBlocking));
+    TRY_OR_CLEAN(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
     TRY_OR_CLEAN(cudaMalloc(&d_states, sbytes));
     TRY_OR_CLEAN(cudaMalloc(&d_out, sbytes));
-    TRY_OR_CLEAN(cudaMalloc(&d_psi, bbytes));
-    TRY_OR_CLEAN(cudaMalloc(&d_hpsi, bbytes));
+    for (int q = 0; q < 2; ++q) {
+        TRY_OR_CLEAN(cudaMalloc(&d_psi[q], bbytes));
+        TRY_OR_CLEAN(cudaMalloc(&d_hpsi[q], bbytes));
+    }
     TRY_OR_CLEAN(cudaMalloc(&d_v, (size_t)m->np * 8));
-    TRY_OR_CLEAN(cudaMemcpyAsync(d_v, vloc_host, (size_t)m->np * 8, cudaMemcpyHostToDevice, st));
-    TRY_OR_CLEAN(cudaMemcpyAsync(d_states, states_host, sbytes, cudaMemcpyHostToDevice, st));
-    for (int ist0 = 0; ist0 < nst_total && rc == RS_OK; ist0 += B) {
-        const int nb = nst_total - ist0 < B ? nst_total - ist0 : B;
-        rc = rs_block_pack(m, d_states, ld, ist0, nb, B, d_psi, dtype, st);
-        if (rc == RS_OK) rc = rs_hamiltonian_apply(m, n, coeffs, d_v, d_psi, d_hpsi, B, dtype, st);
-        if (rc == RS_OK) rc = rs_block_unpack(m, d_hpsi, B, nb, d_out, ld, ist0, dtype, st);
+    TRY_OR_CLEAN(cudaMemcpyAsync(d_v, vloc_host, (size_t)m->np * 8, cudaMemcpyHostToDevice, s_in));
+    for (int k = 0; k < nblocks; ++k) {
+        const int ist0 = k * B, nb = nst_total - ist0 < B ? nst_total - ist0 : B;
+        const size_t off = (size_t)ist0 * ld * esz, bytes = (size_t)nb * ld * esz;
+        TRY_OR_CLEAN(cudaEventCreateWithFlags(&ev_in[k], cudaEventDisableTiming));
+        TRY_OR_CLEAN(cudaEventCreateWithFlags(&ev_cmp[k], cudaEventDisableTiming));
+        TRY_OR_CLEAN(cudaMemcpyAsync((char *)d_states + off, (const char *)states_host + off, bytes, cudaMemcpyHostToDevice, s_in));
+        TRY_OR_CLEAN(cudaEventRecord(ev_in[k], s_in));
+        TRY_OR_CLEAN(cudaStreamWaitEvent(s_cmp, ev_in[k], 0));
+        rc = rs_block_pack(m, d_states, ld, ist0, nb, B, d_psi[k & 1], dtype, s_cmp);
+        if (rc == RS_OK) rc = rs_hamiltonian_apply(m, n, coeffs, d_v, d_psi[k & 1], d_hpsi[k & 1], B, dtype, s_cmp);
+        if (rc == RS_OK) rc = rs_block_unpack(m, d_hpsi[k & 1], B, nb, d_out, ld, ist0, dtype, s_cmp);
+        if (rc != RS_OK) {
+            cudaDeviceSynchronize();
+            cleanup();
+            return rc;
+        }
+        TRY_OR_CLEAN(cudaEventRecord(ev_cmp[k], s_cmp));
+        TRY_OR_CLEAN(cudaStreamWaitEvent(s_out, ev_cmp[k], 0));
+        TRY_OR_CLEAN(cudaMemcpyAsync((char *)hstates_host + off, (const char *)d_out + off, bytes, cudaMemcpyDeviceToHost, s_out));
     }
-    if (rc != RS_OK) {
-        cudaStreamSynchronize(st);
-        cleanup();
-        return rc;
-    }
-    TRY_OR_CLEAN(cudaMemcpyAsync(hstates_host, d_out, sbytes, cudaMemcpyDeviceToHost, st));
-    TRY_OR_CLEAN(cudaStreamSynchronize(st));
+    TRY_OR_CLEAN(cudaStreamSynchronize(s_out));
+    TRY_OR_CLEAN(cudaStreamSynchronize(s_cmp));
+    TRY_OR_CLEAN(cudaStreamSynchronize(s_in));
     cleanup();
 #undef TRY_OR_CLEAN
     return RS_OK;
