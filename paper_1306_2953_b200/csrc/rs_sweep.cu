@@ -252,14 +252,21 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
     uint32_t eparity = 1, rparity = 0;           // the first pass over the stages finds them free
     // V and the indices of a plane are fetched one step (of this group) ahead of their use, so that the
     // global-load latency is not on the per-step path
-    int32_t ci0 = -1, ci1 = -1;
+    // The store offsets of a plane's outputs are needed 4 steps later, when the x arm is complete: this group
+    // staged that plane too (4 is even), so each thread simply remembers its two points' offsets for two of its
+    // own steps and stages them with plane t.
+    uint32_t of0 = 0xffffffffu, of1 = 0xffffffffu;                       // offsets of the plane fetched last (step t)
+    uint32_t ofa0 = 0xffffffffu, ofa1 = 0xffffffffu, ofb0 = 0xffffffffu, ofb1 = 0xffffffffu;   // of steps t - 2, t - 4
     double vv0 = 0.0, vv1 = 0.0;
     auto fetch_v = [&](int slot) {
         const unsigned char *rp = ring + (size_t)slot * SW_REC_BYTES;
-        ci0 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p0 * 4);
-        ci1 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p1 * 4);
+        const int32_t ci0 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p0 * 4);
+        const int32_t ci1 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p1 * 4);
+        const uint32_t coff = *reinterpret_cast<const uint32_t *>(rp + SW_REC_HDR + 4);
         vv0 = ci0 >= 0 ? __ldg(a.vloc + ci0) + w0x3 : 0.0;   // 3 w_0 + V: the whole diagonal coefficient
         vv1 = ci1 >= 0 ? __ldg(a.vloc + ci1) + w0x3 : 0.0;
+        of0 = ci0 >= 0 ? (uint32_t)ci0 * a.ncol + coff : 0xffffffffu;
+        of1 = ci1 >= 0 ? (uint32_t)ci1 * a.ncol + coff : 0xffffffffu;
     };
     if (group < nsteps) {
         mbar_wait(rbar0 + 8u * rs, rparity);
@@ -314,9 +321,11 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         if (hdr.x & HDR_OUTPUT_PLANE) {
             *reinterpret_cast<double *>(sg + v_off0) = vv0;
             *reinterpret_cast<double *>(sg + v_off1) = vv1;
-            *reinterpret_cast<int32_t *>(sg + i_off0) = ci0;
-            *reinterpret_cast<int32_t *>(sg + i_off1) = ci1;
         }
+        *reinterpret_cast<uint32_t *>(sg + i_off0) = ofb0;   // where the outputs of plane t - 4 go
+        *reinterpret_cast<uint32_t *>(sg + i_off1) = ofb1;
+        ofb0 = ofa0, ofb1 = ofa1, ofa0 = of0, ofa1 = of1;
+        of0 = of1 = 0xffffffffu;
         if (gtid == 0) *reinterpret_cast<uint2 *>(sg + SW_HDR_OFF) = make_uint2(hdr.x, hdr.y);
         __syncwarp();
         SW_STAMP(gtid == 0, t, 2);
@@ -358,7 +367,6 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
     // this thread's TMEM lane (its warp's quarter) and the column range of its warp
     const uint32_t tbase = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(warp >> 2) * 192u;
     const uint32_t t_in = tbase;          // [patch row j][slot t mod 4][i]: centre values of the last 4 planes (doubles)
-    const uint32_t t_ix = tbase + 128u;   // [slot t mod 4][16]: store offsets of the last 4 planes' outputs
 
     const uint32_t b0 = (uint32_t)(((N + 4 * py) * SW_W + 4 * pz) * SW_SLOT_BYTES + c * 8);   // patch row 0, window slot 0
     const uint32_t vrow = (uint32_t)((py * SW_W) * SW_SLOT_BYTES + (4 * pz) * 8);
@@ -371,14 +379,6 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
         for (int j = 0; j < 4; ++j)
 #pragma unroll
             for (int i = 0; i < 4; ++i) acc[k][j][i] = 0.0;
-    {   // no pending output yet: all parked offsets invalid
-        uint32_t inv[16];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) inv[q] = 0xffffffffu;
-#pragma unroll
-        for (int k = 0; k < N; ++k) tm_st16(t_ix + k * 16, inv);
-    }
-
     int stage = 0;
     uint32_t parity = 0;
     const double w0x3 = 3.0 * w.w[0];
@@ -389,10 +389,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
         for (int PH = 0; PH < N; ++PH) {
             const int t = t0 + PH;
             if (t >= nsteps) break;
-            // store offsets of the outputs this step completes (plane t - 4); in flight during the wait
             tm_wait_st();
-            uint32_t io[16];
-            tm_ld16(t_ix + PH * 16, io);
             SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 4);
             mbar_wait(full0 + 8u * stage, parity);
             SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 5);
@@ -401,22 +398,13 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             const int mode = (int)((hdr.x >> (2 * warp)) & 3u);
             const double *pb = reinterpret_cast<const double *>(sp + b0);
 
-            uint32_t in_[16];   // this plane's store offsets, parked for 4 steps
-            if (mode == MODE_FULL) {
+            // store offsets of the outputs this step completes (plane t - 4), staged by the producer; -1: none
+            uint32_t io[16];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int4 q = *reinterpret_cast<const int4 *>(sp + irow + j * 64);
-                    const int qq[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-                        in_[4 * j + i] = qq[i] >= 0 ? (uint32_t)qq[i] * a.ncol + hdr.y : 0xffffffffu;
-                }
-            } else {
-#pragma unroll
-                for (int q = 0; q < 16; ++q) in_[q] = 0xffffffffu;
+            for (int j = 0; j < 4; ++j) {
+                const uint4 q = *reinterpret_cast<const uint4 *>(sp + irow + j * 64);
+                io[4 * j] = q.x, io[4 * j + 1] = q.y, io[4 * j + 2] = q.z, io[4 * j + 3] = q.w;
             }
-            tm_wait_ld16(io);
-            tm_st16(t_ix + PH * 16, in_);
 
             if (mode == MODE_FULL) {
                 double ctr[4][4];
@@ -539,7 +527,9 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     __shared__ uint64_t rec_bar[SW_RING];
     __shared__ uint32_t tmem_base_s;
 
-    const int tid = threadIdx.x, warp = tid >> 5;
+    // threads 0..255: the 8 producer warps; threads 256..511: the 8 consumer warps (the higher warp ids, which the
+    // warp scheduler favours when several warps are ready)
+    const int tid = threadIdx.x, ctid = tid - (SW_THREADS - SW_CONSUMERS), warp = tid >> 5;
     const int2 item = a.items[blockIdx.x];
     const int nsteps = item.y;
     const long long clock0 = clock64();
@@ -554,7 +544,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
         for (int s = 0; s < SW_RING; ++s) mbar_init(smem_u32(&rec_bar[s]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    if (warp == 0) {
+    if (warp == (SW_THREADS - SW_CONSUMERS) / 32) {   // first consumer warp
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_base_s)),
                      "n"(SW_TMEM_COLS)
                      : "memory");
@@ -564,18 +554,18 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
 
-    // register re-split: 512 x 128 at launch = 256 x 24 (producers) + 256 x 232 (consumers); the pool that
+    // register re-split: 512 x 128 at launch = 256 x 32 (producers) + 256 x 224 (consumers); the pool that
     // setmaxnreg.inc draws from holds only what setmaxnreg.dec released, so the two must balance exactly
-    if (tid >= SW_CONSUMERS) {
+    if (ctid < 0) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 32;\n");
         sweep_producer<TENSOR>(a, maps, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), smem_u32(&rec_bar[0]),
-                               a.recs + (size_t)item.x * SW_REC_BYTES, nsteps, tid - SW_CONSUMERS, 3.0 * w.w[0]);
+                               a.recs + (size_t)item.x * SW_REC_BYTES, nsteps, tid, 3.0 * w.w[0]);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;\n");
-        sweep_consumer(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, tid);
+        sweep_consumer(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid);
         named_bar_sync(1, SW_CONSUMERS);
-        if (tid == 0 && a.cycles) a.cycles[blockIdx.x] = clock64() - clock0;
-        if (warp == 0)
+        if (ctid == 0 && a.cycles) a.cycles[blockIdx.x] = clock64() - clock0;
+        if (ctid < 32)
             asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base_s), "n"(SW_TMEM_COLS) : "memory");
     }
 }
