@@ -149,8 +149,7 @@ __device__ __forceinline__ void tm_ld32(uint32_t taddr, uint32_t (&r)[32])
 }
 __device__ __forceinline__ void tm_st8(uint32_t taddr, const uint32_t (&r)[8])
 {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};\n" ::"r"(taddr), R4(r, 0), R4(r, 4)
-                 : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};\n" ::"r"(taddr), R4(r, 0), R4(r, 4));
 }
 __device__ __forceinline__ void tm_st16(uint32_t taddr, const uint32_t (&r)[16])
 {
@@ -162,14 +161,14 @@ __device__ __forceinline__ void tm_st16(uint32_t taddr, const uint32_t (&r)[16])
 // The loaded registers are passed through the wait so that no use of them can be scheduled above it.
 __device__ __forceinline__ void tm_wait_ld16(uint32_t (&r)[16])
 {
-    asm volatile("tcgen05.wait::ld.sync.aligned;\n" : P4(r, 0), P4(r, 4), P4(r, 8), P4(r, 12)::"memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" : P4(r, 0), P4(r, 4), P4(r, 8), P4(r, 12));
 }
 __device__ __forceinline__ void tm_wait_ld32(uint32_t (&r)[32])
 {
     asm volatile("tcgen05.wait::ld.sync.aligned;\n"
-                 : P4(r, 0), P4(r, 4), P4(r, 8), P4(r, 12), P4(r, 16), P4(r, 20), P4(r, 24), P4(r, 28)::"memory");
+                 : P4(r, 0), P4(r, 4), P4(r, 8), P4(r, 12), P4(r, 16), P4(r, 20), P4(r, 24), P4(r, 28));
 }
-__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n"); }
 #undef R4
 #undef W4
 #undef P4
@@ -183,10 +182,9 @@ __device__ __forceinline__ void store_if_valid(double *base, uint32_t off, doubl
         ".reg .u64 q;\n"
         "setp.ne.u32 p, %0, 0xffffffff;\n"
         "mad.wide.u32 q, %0, 8, %1;\n"
-        "@p st.global.f64 [q], %2;\n"
+        "@p st.global.cs.f64 [q], %2;\n"
         "}\n" ::"r"(off),
-        "l"(base), "d"(v)
-        : "memory");
+        "l"(base), "d"(v));   // no "memory" clobber: the compiler may move shared-memory loads across these stores
 }
 
 __device__ __forceinline__ double words2double(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
@@ -379,6 +377,9 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
         for (int j = 0; j < 4; ++j)
 #pragma unroll
             for (int i = 0; i < 4; ++i) acc[k][j][i] = 0.0;
+#if SW_EXP & 16
+    if (warp >= 4) __nanosleep(700);   // experiment: start the second warp of each scheduler half a step late
+#endif
     int stage = 0;
     uint32_t parity = 0;
     const double w0x3 = 3.0 * w.w[0];
