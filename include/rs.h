@@ -68,7 +68,7 @@ typedef enum {
     RS_KERNEL_AUTO = 0,   /* best available for this mesh / order / width                         */
     RS_KERNEL_GATHER = 1, /* per-point neighbour table, one gathered load per star arm (any mesh) */
     RS_KERNEL_SWEEP = 2   /* plane-sweep kernel: smem-staged planes + register x-window (RS_ORDER_LEX,
-                             non-periodic mesh, fd_order 4, 16 | 32 | 64 | 128 real columns)       */
+                             non-periodic mesh, fd_order 4 or 6, 16 | 32 | 64 | 128 real columns)  */
 } rs_kernel;
 
 #define RS_MAX_FD_ORDER 8
@@ -148,7 +148,8 @@ int rs_version(void);
 /* Tuning knobs for tests and ablations (not needed for normal use); they take effect for tables built
  * afterwards.  "sweep_planes": x-slab thickness of a plane-sweep work item (default 32); "sweep_ctas":
  * number of persistent CTAs (0 = one per SM); "sweep_tensor": 1 = use the 2-D tensor-map copies also for
- * 16-column blocks.  Unknown name -> RS_ERR_INVALID_ARG.                                               */
+ * 16-column blocks; "sweep_shape": 1 = run fd_order 4 on the experimental 12-warp kernel shape.
+ * Unknown name -> RS_ERR_INVALID_ARG.                                                                  */
 rs_status rs_set_tuning(const char *name, int value);
 /* Host-only diagnostic (no device needed): build the plane-sweep kernel's compact records for (mesh,
  * fd_order, block width nst of dtype) dealt to `nctas` CTAs with slabs of `max_planes`, replay them

@@ -27,14 +27,14 @@ constexpr int RS_BRICK_PTS = RS_BRICK * RS_BRICK * RS_BRICK;  // 64 points
 //                           bytes copied (2-D tensor boxes)};
 //   cidx[256]              mesh index of the tile's own points (-1: outside the mesh / not an output plane).
 #define RS_SWEEP_MAXRUN 64
-#define RS_SWEEP_REC_BYTES (RS_SWEEP_MAXRUN * 8 + 80 + 16 + 256 * 4)   // runs | fill | hdr | cidx, packed
 struct rs_sweep_piece {
     int iy, iz, xa, xb, chunk;   // tile, output planes [xa, xb), column slice
 };
 struct rs_sweep_host {
     std::vector<int2> items;                         // per CTA: {first record, number of steps}
     std::vector<std::vector<rs_sweep_piece>> pieces; // per CTA, in execution order
-    std::vector<unsigned char> recs;                 // [nrec][RS_SWEEP_REC_BYTES]
+    std::vector<unsigned char> recs;                 // [nrec][rec_bytes]
+    int rec_bytes = 0;                               // 608 + 4 per tile point (depends on the kernel shape)
     int64_t nrec = 0;
     std::vector<double> load;                        // modelled load per CTA
     double cost_max = 0.0, cost_mean = 0.0;          // modelled load of the busiest / average CTA
@@ -42,6 +42,7 @@ struct rs_sweep_host {
 struct rs_sweep_tables {
     bool ok = false;              // false: some plane needs more than RS_SWEEP_MAXRUN runs (use the gather kernel)
     int64_t nitems = 0, nrec = 0, bytes = 0;
+    int variant = 0;              // which compiled kernel shape the records were built for
     int2 *d_items = nullptr;
     unsigned char *d_recs = nullptr;
     long long *d_cycles = nullptr;                   // per CTA: clock ticks of the last launch

@@ -31,8 +31,11 @@
 //     store) and a 2-bit mode per warp (empty / centre-only / full) that lets a warp skip the planes
 //     in which its 4 x 8 region holds no mesh point.  The records expand to exactly the plain table of
 //     rs_mesh_get_index_map (reading S15; rs_sweep_selfcheck verifies this on the host).
+// The kernel is a template over its shape (star half-width, tile height, patch height, producer groups):
+// fd_order 4 runs 16 x 16 tiles with 4 x 4 patches, fd_order 6 runs 8 x 16 tiles with 2 x 4 patches (6 pending
+// planes of a 4 x 4 patch do not fit the register file).  The text below describes the fd_order 4 shape.
 // Requires RS_ORDER_LEX (in-domain points of a z-row consecutive in memory), a non-periodic mesh,
-// fd_order 4 and a block of 16, 32, 64 or 128 real columns; anything else is served by the gather kernel.
+// fd_order 4 or 6 and a block of 16, 32, 64 or 128 real columns; anything else is served by the gather kernel.
 #include <cuda.h>
 
 #include <algorithm>
@@ -42,29 +45,65 @@
 
 namespace {
 
-constexpr int SW_N = 4;                  // half-width of the star
-constexpr int SW_T = 16;                 // tile edge (points) in y and z
-constexpr int SW_W = SW_T + 2 * SW_N;    // 24: rows / z-slots of a staged plane
+constexpr int SW_TZ = 16;                // tile edge (points) in z: one copy run per z-row
+constexpr int SW_PZ = 4;                 // patch width in z: 4 patches across the tile
 constexpr int SW_C = 16;                 // columns per CTA
 constexpr int SW_SLOT_BYTES = SW_C * 8;  // 128
-constexpr int SW_STAGE_BYTES = SW_W * SW_W * SW_SLOT_BYTES;  // 73,728: uniform [24][24] slots; corners hold V, idx, header
 constexpr int SW_STAGES = 3;
-constexpr int SW_CONSUMERS = 256;        // 8 consumer warps
-constexpr int SW_THREADS = 512;          // + two producer warpgroups (steps alternate between them)
 constexpr int SW_MAXRUN = RS_SWEEP_MAXRUN;
-constexpr int SW_TMEM_COLS = 512;        // allocated; used: 2 x (4 x 32 [centre ring] + 4 x 16 [offset ring])
-// packed per-plane record (rs_internal.h): runs | fill rows | header | indices of the tile's points
+constexpr int SW_TMEM_COLS = 512;
+// packed per-plane record (rs_internal.h): runs | fill bitmap | header | indices of the tile's points
 constexpr int SW_REC_RUNS = 0, SW_REC_FILL = SW_MAXRUN * 8, SW_REC_HDR = SW_REC_FILL + 80, SW_REC_CIDX = SW_REC_HDR + 16;
-constexpr int SW_REC_BYTES = RS_SWEEP_REC_BYTES;
-static_assert(SW_REC_BYTES == SW_REC_CIDX + 256 * 4 && SW_REC_BYTES % 16 == 0, "record layout");
-constexpr int SW_RING = 6;               // record ring of the producer group
+constexpr int SW_RING = 6;               // record ring of the producers
 constexpr int SW_LOOKAHEAD = 3;          // records are requested this many steps ahead (SW_RING >= SW_LOOKAHEAD + 3)
-constexpr size_t SW_SMEM = (size_t)SW_STAGES * SW_STAGE_BYTES + (size_t)SW_RING * SW_REC_BYTES;
-static_assert(SW_SMEM + 256 <= 232448, "shared memory budget");
-constexpr int SW_NBOX = 6;               // tensor-map box heights 1, 2, 4, 8, 16, 24
+constexpr int SW_NBOX = 6;               // tensor-map box heights 1, 2, 4, 8, 16, 24 (a run of 25..28 points takes two boxes)
+
+// Kernel shape: star half-width N, tile of TY x 16 (y, z) points, register patch of PY x 4 points per thread,
+// NGROUPS producer groups of 4 warps.  Compiled shapes (rs_sweep_variant()):
+//   <4, 16, 4, 2>  the default for fd_order 4: 8 consumer warps, 16 outputs per thread, 4 pending planes in registers
+//   <6,  8, 2, 2>  fd_order 6: 6 pending planes of a 4 x 4 patch do not fit the register file; 2 x 4 patches do
+//   <4, 12, 2, 1>  experiment for fd_order 4: 12 lighter consumer warps (rs_set_tuning("sweep_shape", 1))
+template <int N_, int TY_, int PY_, int NGROUPS_>
+struct sweep_shape {
+    static constexpr int N = N_, TY = TY_, PY = PY_, NGROUPS = NGROUPS_;
+    static constexpr int WY = TY + 2 * N, WZ = SW_TZ + 2 * N;            // rows / z-slots of a staged plane
+    static constexpr int STAGE_BYTES = WY * WZ * SW_SLOT_BYTES;         // uniform [WY][WZ] slots; the corners hold V, offsets, header
+    static constexpr int NPT = TY * SW_TZ;                              // tile points
+    static constexpr int CONSUMERS = (TY / PY) * (SW_TZ / SW_PZ) * SW_C;   // one thread per (patch, column)
+    static constexpr int NCW = CONSUMERS / 32;
+    static constexpr int PRODUCERS = 128 * NGROUPS;
+    static constexpr int THREADS = PRODUCERS + CONSUMERS;
+    static constexpr int REC_BYTES = SW_REC_CIDX + NPT * 4;
+    static constexpr int ROW_WORDS = N * 2 * SW_PZ;                      // tensor memory: one patch row = N ring slots x 4 doubles
+    static constexpr size_t SMEM = (size_t)SW_STAGES * STAGE_BYTES + (size_t)SW_RING * REC_BYTES;
+    // corner B (rows 0.., slots WZ-N..): the store offsets (4 tile rows = 256 bytes per corner row), then the header
+    static constexpr uint32_t HDR_OFF = (uint32_t)(WZ - N + 2) * SW_SLOT_BYTES;
+    // registers: THREADS x LAUNCH_REGS at launch = PRODUCERS x PROD_REGS + CONSUMERS x CONS_REGS at most
+    static constexpr int LAUNCH_REGS = (65536 / THREADS) & ~7;
+    static constexpr int PROD_REGS = 32;
+    static constexpr int CONS_REGS = (LAUNCH_REGS + (LAUNCH_REGS - PROD_REGS) * PRODUCERS / CONSUMERS) & ~7;
+    static_assert(TY % PY == 0 && 4 % PY == 0 && CONSUMERS % 128 == 0 && N % NGROUPS == 0, "shape");
+    static_assert(TY <= 4 * N && N >= 4, "the corners must hold V (512 bytes per corner row) and the offsets");
+    static_assert(REC_BYTES % 16 == 0 && SMEM + 256 <= 232448, "shared memory budget");
+    static_assert((NCW + 3) / 4 * PY * ROW_WORDS <= SW_TMEM_COLS, "tensor memory budget");
+    static_assert(WY * WZ <= 18 * 32, "zero-fill bitmap");
+};
+using shape_n4 = sweep_shape<4, 16, 4, 2>;
+using shape_n6 = sweep_shape<6, 8, 2, 2>;
+using shape_n4w12 = sweep_shape<4, 12, 2, 1>;
+
+// the same numbers at run time, for the host-side builder
+struct shape_rt {
+    int N, TY, PY, WY, WZ, NPT, NCW, rec_bytes;
+};
+template <class S>
+shape_rt shape_of()
+{
+    return shape_rt{S::N, S::TY, S::PY, S::WY, S::WZ, S::NPT, S::NCW, S::REC_BYTES};
+}
 
 enum { MODE_EMPTY = 0, MODE_CENTRE = 1, MODE_FULL = 2 };
-constexpr uint32_t HDR_OUTPUT_PLANE = 1u << 16;   // the plane has outputs: stage V and the indices
+constexpr uint32_t HDR_OUTPUT_PLANE = 1u << 31;   // the plane has outputs: stage V and the indices (bits 0..23: 2 per warp)
 
 // ---------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -74,10 +113,6 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)_
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.expect_tx.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
@@ -151,13 +186,6 @@ __device__ __forceinline__ void tm_st8(uint32_t taddr, const uint32_t (&r)[8])
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};\n" ::"r"(taddr), R4(r, 0), R4(r, 4));
 }
-__device__ __forceinline__ void tm_st16(uint32_t taddr, const uint32_t (&r)[16])
-{
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};\n" ::"r"(taddr),
-        R4(r, 0), R4(r, 4), R4(r, 8), R4(r, 12)
-        : "memory");
-}
 // The loaded registers are passed through the wait so that no use of them can be scheduled above it.
 __device__ __forceinline__ void tm_wait_ld16(uint32_t (&r)[16])
 {
@@ -194,7 +222,7 @@ __device__ __forceinline__ double words2double(uint32_t lo, uint32_t hi) { retur
 // ---------------------------------------------------------------------------------------------
 struct sweep_args {
     const int2 *items;           // per CTA: {first record, number of steps}
-    const unsigned char *recs;   // [nrec][SW_REC_BYTES] packed per-plane records
+    const unsigned char *recs;   // [nrec][REC_BYTES] packed per-plane records
     const double *vloc;
     const double *psi;
     double *hpsi;
@@ -204,9 +232,6 @@ struct sweep_args {
 struct sweep_maps {
     CUtensorMap box[SW_NBOX];    // psi as a [np+1][ncol] fp64 tensor, box {16, 1|2|4|8|16|24}
 };
-
-// stage offsets of the small per-plane arrays kept in the unused corners of the [24][24] slot grid
-constexpr uint32_t SW_HDR_OFF = (uint32_t)((SW_W - SW_N) * SW_W) * SW_SLOT_BYTES;   // corner C: row 20, slot 0
 
 // Optional timeline of one CTA (development builds only, -DSW_TRACE): clock64 stamps per step after the per-CTA ticks.
 #ifndef SW_EXP
@@ -218,65 +243,73 @@ constexpr uint32_t SW_HDR_OFF = (uint32_t)((SW_W - SW_N) * SW_W) * SW_SLOT_BYTES
 #define SW_STAMP(cond, t, k) do { } while (0)
 #endif
 
-// ---- producer warps: two groups of 4 warps stage plane after plane, group g taking steps t = g (mod 2) ------
-// Inside a group every warp takes a quarter of each job (copy runs, zero fill, V / index gather) and arrives
+// ---- producer warps: NGROUPS groups of 4 warps stage plane after plane, group g taking steps t = g (mod NGROUPS) ----
+// Inside a group every warp takes a quarter of each job (copy runs, zero fill, V / offset staging) and arrives
 // once on the stage's "full" barrier.  Two groups because a step's chain of barrier waits, copy issues and
 // fences is latency-bound (~2000 clocks measured): two steps in flight double the rate.  Records arrive through
 // a ring of SW_RING slots; the group working on step t requests record t + SW_LOOKAHEAD: having passed the
 // "empty" wait of step t proves that the consumers, hence all producer warps, finished step t - 3, whose slot
 // is the one overwritten.
-template <bool TENSOR>
+template <class S, bool TENSOR>
 __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_maps &maps, unsigned char *smem,
                                                uint32_t full0, uint32_t empty0, uint32_t rbar0, const unsigned char *recs,
                                                int nsteps, int ptid, double w0x3)
 {
-    constexpr int N = SW_N;
+    constexpr int N = S::N, G = S::NGROUPS;
+    constexpr int PPT = (S::NPT + 127) / 128;   // tile points per thread (V and offsets)
+    constexpr int HS = N / G;                   // a plane's store offsets are staged HS own steps after the plane itself
     const int group = ptid >> 7, gtid = ptid & 127, lane = ptid & 31, pw = gtid >> 5;
-    unsigned char *const ring = smem + (size_t)SW_STAGES * SW_STAGE_BYTES;
+    unsigned char *const ring = smem + (size_t)SW_STAGES * S::STAGE_BYTES;
     const uint32_t sbase = smem_u32(smem);
     auto request_rec = [&](int r) {   // one thread; preceded by a fence.proxy.async of that thread
         const uint32_t bar = rbar0 + 8u * (r % SW_RING);
-        mbar_arrive_expect_tx(bar, SW_REC_BYTES);
-        bulk_g2s(smem_u32(ring) + (uint32_t)(r % SW_RING) * SW_REC_BYTES, recs + (size_t)r * SW_REC_BYTES, SW_REC_BYTES, bar);
+        mbar_arrive_expect_tx(bar, S::REC_BYTES);
+        bulk_g2s(smem_u32(ring) + (uint32_t)(r % SW_RING) * S::REC_BYTES, recs + (size_t)r * S::REC_BYTES, S::REC_BYTES, bar);
     };
     if (ptid == 0)
         for (int r = 0; r < SW_LOOKAHEAD && r < nsteps; ++r) request_rec(r);
-    // this thread's jobs: copy run `myrun` (lanes 0..15 of each warp), fill slots gtid + 128 k, tile points gtid and gtid + 128
+    // this thread's jobs: copy run `myrun` (lanes 0..15 of each warp), a share of the zero fill, tile points gtid (+ 128)
     const int myrun = lane * 4 + pw;
-    const int p0 = gtid, p1 = gtid + 128;
-    const uint32_t v_off0 = (uint32_t)(((p0 >> 6) * SW_W) * SW_SLOT_BYTES + (p0 & 63) * 8), v_off1 = v_off0 + 2 * SW_W * SW_SLOT_BYTES;
-    const uint32_t i_off0 = (uint32_t)(((p0 >> 6) * SW_W + SW_W - N) * SW_SLOT_BYTES + (p0 & 63) * 4), i_off1 = i_off0 + 2 * SW_W * SW_SLOT_BYTES;
-    int stage = group, rs = group;               // t mod SW_STAGES, t mod SW_RING
-    uint32_t eparity = 1, rparity = 0;           // the first pass over the stages finds them free
-    // V and the indices of a plane are fetched one step (of this group) ahead of their use, so that the
-    // global-load latency is not on the per-step path
-    // The store offsets of a plane's outputs are needed 4 steps later, when the x arm is complete: this group
-    // staged that plane too (4 is even), so each thread simply remembers its two points' offsets for two of its
-    // own steps and stages them with plane t.
-    uint32_t of0 = 0xffffffffu, of1 = 0xffffffffu;                       // offsets of the plane fetched last (step t)
-    uint32_t ofa0 = 0xffffffffu, ofa1 = 0xffffffffu, ofb0 = 0xffffffffu, ofb1 = 0xffffffffu;   // of steps t - 2, t - 4
-    double vv0 = 0.0, vv1 = 0.0;
+    // point p = (ty, tz): V at corner A row ty / 4, offsets at corner B row ty / 4 (4 tile rows per corner row)
+    const uint32_t v_off0 = (uint32_t)(((gtid >> 6) * S::WZ) * SW_SLOT_BYTES + (gtid & 63) * 8);
+    const uint32_t i_off0 = (uint32_t)(((gtid >> 6) * S::WZ + S::WZ - N) * SW_SLOT_BYTES + (gtid & 63) * 4);
+    constexpr uint32_t NEXT_POINT = 2 * S::WZ * SW_SLOT_BYTES;   // point gtid + 128: two corner rows further
+    int stage = group % SW_STAGES, rs = group % SW_RING;   // t mod SW_STAGES, t mod SW_RING
+    uint32_t eparity = 1, rparity = 0;                     // the first pass over the stages finds them free
+    // V and the offsets of a plane are fetched one own step ahead of their use, so that the global-load latency is
+    // not on the per-step path.  The store offsets of a plane's outputs are needed N steps later, when the x arm is
+    // complete: this group staged that plane too (N is a multiple of the number of groups), so each thread simply
+    // remembers its points' offsets for HS of its own steps and stages them with plane t.
+    double vv[PPT];
+    uint32_t of[PPT], hist[HS][PPT];
+#pragma unroll
+    for (int q = 0; q < PPT; ++q) {
+        vv[q] = 0.0, of[q] = 0xffffffffu;
+#pragma unroll
+        for (int h = 0; h < HS; ++h) hist[h][q] = 0xffffffffu;
+    }
     auto fetch_v = [&](int slot) {
-        const unsigned char *rp = ring + (size_t)slot * SW_REC_BYTES;
-        const int32_t ci0 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p0 * 4);
-        const int32_t ci1 = *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p1 * 4);
+        const unsigned char *rp = ring + (size_t)slot * S::REC_BYTES;
         const uint32_t coff = *reinterpret_cast<const uint32_t *>(rp + SW_REC_HDR + 4);
-        vv0 = ci0 >= 0 ? __ldg(a.vloc + ci0) + w0x3 : 0.0;   // 3 w_0 + V: the whole diagonal coefficient
-        vv1 = ci1 >= 0 ? __ldg(a.vloc + ci1) + w0x3 : 0.0;
-        of0 = ci0 >= 0 ? (uint32_t)ci0 * a.ncol + coff : 0xffffffffu;
-        of1 = ci1 >= 0 ? (uint32_t)ci1 * a.ncol + coff : 0xffffffffu;
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) {
+            const int p = gtid + 128 * q;
+            const int32_t ci = p < S::NPT ? *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p * 4) : -1;
+            vv[q] = ci >= 0 ? __ldg(a.vloc + ci) + w0x3 : 0.0;   // 3 w_0 + V: the whole diagonal coefficient
+            of[q] = ci >= 0 ? (uint32_t)ci * a.ncol + coff : 0xffffffffu;
+        }
     };
     if (group < nsteps) {
         mbar_wait(rbar0 + 8u * rs, rparity);
         fetch_v(rs);
     }
-    for (int t = group; t < nsteps; t += 2) {
+    for (int t = group; t < nsteps; t += G) {
         SW_STAMP(gtid == 0, t, 0);
         // everything the copies need is read from the record (present: fetch_v waited for it) BEFORE the wait for
         // the stage, so that the copies leave right after the consumers release it
-        const unsigned char *rp = ring + (size_t)rs * SW_REC_BYTES;
-        const uint32_t sb = sbase + (uint32_t)stage * SW_STAGE_BYTES;
-        unsigned char *const sg = smem + (size_t)stage * SW_STAGE_BYTES;
+        const unsigned char *rp = ring + (size_t)rs * S::REC_BYTES;
+        const uint32_t sb = sbase + (uint32_t)stage * S::STAGE_BYTES;
+        unsigned char *const sg = smem + (size_t)stage * S::STAGE_BYTES;
         const uint32_t bar = full0 + 8u * stage;
         const uint4 hdr = *reinterpret_cast<const uint4 *>(rp + SW_REC_HDR);   // {modes|flags, column offset, tx bytes 1-D, tx bytes 2-D}
         uint2 run = make_uint2(0u, 0u);
@@ -300,11 +333,10 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         }
         if (gtid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
         SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 4);
-        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 5);
-        // ---- zero fill: bit s of the record's bitmap says that slot s of the [24][24] grid must be cleared.  A warp
+        // ---- zero fill: bit s of the record's bitmap says that slot s of the [WY][WZ] grid must be cleared.  A warp
         //      takes every 4th word of the bitmap; a quarter-warp clears one slot with 8 conflict-free 16-byte stores ----
 #pragma unroll 1
-        for (int wd = pw; wd < (SW_W * SW_W + 31) / 32; wd += 4) {
+        for (int wd = pw; wd < (S::WY * S::WZ + 31) / 32; wd += 4) {
             const uint32_t m = *reinterpret_cast<const uint32_t *>(rp + SW_REC_FILL + wd * 4);
             if (m == 0) continue;
 #pragma unroll 1
@@ -315,16 +347,19 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
                     *reinterpret_cast<float4 *>(sg + (size_t)sl * SW_SLOT_BYTES + (lane & 7) * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
-        // ---- V and the mesh indices of the tile's own points (output planes only) ----------------------
-        if (hdr.x & HDR_OUTPUT_PLANE) {
-            *reinterpret_cast<double *>(sg + v_off0) = vv0;
-            *reinterpret_cast<double *>(sg + v_off1) = vv1;
+        // ---- V of the tile's own points (output planes only) and the store offsets of plane t - N ------------
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) {
+            if (gtid + 128 * q < S::NPT) {
+                if (hdr.x & HDR_OUTPUT_PLANE) *reinterpret_cast<double *>(sg + v_off0 + q * NEXT_POINT) = vv[q];
+                *reinterpret_cast<uint32_t *>(sg + i_off0 + q * NEXT_POINT) = hist[HS - 1][q];
+            }
+#pragma unroll
+            for (int h = HS - 1; h > 0; --h) hist[h][q] = hist[h - 1][q];
+            hist[0][q] = of[q];
+            of[q] = 0xffffffffu;
         }
-        *reinterpret_cast<uint32_t *>(sg + i_off0) = ofb0;   // where the outputs of plane t - 4 go
-        *reinterpret_cast<uint32_t *>(sg + i_off1) = ofb1;
-        ofb0 = ofa0, ofb1 = ofa1, ofa0 = of0, ofa1 = of1;
-        of0 = of1 = 0xffffffffu;
-        if (gtid == 0) *reinterpret_cast<uint2 *>(sg + SW_HDR_OFF) = make_uint2(hdr.x, hdr.y);
+        if (gtid == 0) *reinterpret_cast<uint2 *>(sg + S::HDR_OFF) = make_uint2(hdr.x, hdr.y);
         __syncwarp();
         SW_STAMP(gtid == 0, t, 2);
         // one arrival per warp; the group's first thread also announces the bytes of all the group's copies (the
@@ -336,17 +371,17 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
                 mbar_arrive(bar);
         }
         SW_STAMP(gtid == 0, t, 3);
-        stage += 2;
-        if (stage >= SW_STAGES) {
+        stage += G;
+        if (stage >= SW_STAGES) {   // G <= SW_STAGES: at most one wrap
             stage -= SW_STAGES;
             eparity ^= 1u;
         }
-        rs += 2;
+        rs += G;
         if (rs >= SW_RING) {
             rs -= SW_RING;
             rparity ^= 1u;
         }
-        if (t + 2 < nsteps) {   // this group's next step: its record was requested SW_LOOKAHEAD steps before it
+        if (t + G < nsteps) {   // this group's next step: its record was requested SW_LOOKAHEAD steps before it
             mbar_wait(rbar0 + 8u * rs, rparity);
             SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 6);
             fetch_v(rs);
@@ -356,33 +391,55 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
 }
 
 // ---- consumer warps: the arithmetic ----------------------------------------------------------------
+// tensor memory, one patch row: [ring slot t mod N][4 doubles]; loaded whole (N x 8 words), stored one slot at a time
+template <int N>
+__device__ __forceinline__ void tm_ld_row(uint32_t taddr, uint32_t (&r)[N * 8])
+{
+    static_assert(N == 4 || N == 6, "tensor-memory row shapes");
+    uint32_t(&lo)[32] = reinterpret_cast<uint32_t(&)[32]>(r[0]);
+    tm_ld32(taddr, lo);
+    if constexpr (N == 6) {
+        uint32_t(&hi)[16] = reinterpret_cast<uint32_t(&)[16]>(r[32]);
+        tm_ld16(taddr + 32, hi);
+    }
+}
+template <int N>
+__device__ __forceinline__ void tm_wait_row(uint32_t (&r)[N * 8])
+{
+    uint32_t(&lo)[32] = reinterpret_cast<uint32_t(&)[32]>(r[0]);
+    if constexpr (N == 6) {
+        uint32_t(&hi)[16] = reinterpret_cast<uint32_t(&)[16]>(r[32]);
+        tm_wait_ld16(hi);
+    }
+    tm_wait_ld32(lo);
+}
+
+template <class S>
 __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_weights &w, const unsigned char *smem,
                                                uint32_t full0, uint32_t empty0, uint32_t tmem_base, int nsteps, int tid)
 {
-    constexpr int N = SW_N;
+    constexpr int N = S::N, PY = S::PY, PZ = SW_PZ, WZ = S::WZ;
     const int lane = tid & 31, warp = tid >> 5;
     const int c = tid & 15, patch = tid >> 4, py = patch >> 2, pz = patch & 3;
-    // this thread's TMEM lane (its warp's quarter) and the column range of its warp
-    const uint32_t tbase = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(warp >> 2) * 192u;
-    const uint32_t t_in = tbase;          // [patch row j][slot t mod 4][i]: centre values of the last 4 planes (doubles)
+    const int ty0 = PY * py;   // first tile row of the patch
+    // this thread's TMEM lane (its warp's quarter) and the column range of its warp:
+    // [patch row j][ring slot t mod N][i]: centre values of the last N planes (doubles)
+    const uint32_t t_in = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(warp >> 2) * (PY * S::ROW_WORDS);
 
-    const uint32_t b0 = (uint32_t)(((N + 4 * py) * SW_W + 4 * pz) * SW_SLOT_BYTES + c * 8);   // patch row 0, window slot 0
-    const uint32_t vrow = (uint32_t)((py * SW_W) * SW_SLOT_BYTES + (4 * pz) * 8);
-    const uint32_t irow = (uint32_t)((py * SW_W + SW_W - N) * SW_SLOT_BYTES + (4 * pz) * 4);
+    const uint32_t b0 = (uint32_t)(((N + ty0) * WZ + PZ * pz) * SW_SLOT_BYTES + c * 8);   // patch row 0, window slot 0
+    // V (corner A) and store offsets (corner B): 4 tile rows per corner row, PY divides 4
+    const uint32_t vrow = (uint32_t)(((ty0 >> 2) * WZ) * SW_SLOT_BYTES + ((ty0 & 3) * SW_TZ + PZ * pz) * 8);
+    const uint32_t irow = (uint32_t)(((ty0 >> 2) * WZ + WZ - N) * SW_SLOT_BYTES + ((ty0 & 3) * SW_TZ + PZ * pz) * 4);
 
-    double acc[N][4][4];   // pending outputs: acc[t mod 4] belongs to plane t
+    double acc[N][PY][PZ];   // pending outputs: acc[t mod N] belongs to plane t
 #pragma unroll
     for (int k = 0; k < N; ++k)
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < PY; ++j)
 #pragma unroll
-            for (int i = 0; i < 4; ++i) acc[k][j][i] = 0.0;
-#if SW_EXP & 16
-    if (warp >= 4) __nanosleep(700);   // experiment: start the second warp of each scheduler half a step late
-#endif
+            for (int i = 0; i < PZ; ++i) acc[k][j][i] = 0.0;
     int stage = 0;
     uint32_t parity = 0;
-    const double w0x3 = 3.0 * w.w[0];
     double *const hp = a.hpsi + c;
 
     for (int t0 = 0; t0 < nsteps; t0 += N) {
@@ -394,37 +451,38 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 4);
             mbar_wait(full0 + 8u * stage, parity);
             SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 5);
-            const unsigned char *sp = smem + (size_t)stage * SW_STAGE_BYTES;
-            const uint2 hdr = *reinterpret_cast<const uint2 *>(sp + SW_HDR_OFF);   // {modes | flags, column offset}
+            const unsigned char *sp = smem + (size_t)stage * S::STAGE_BYTES;
+            const uint2 hdr = *reinterpret_cast<const uint2 *>(sp + S::HDR_OFF);   // {modes | flags, column offset}
             const int mode = (int)((hdr.x >> (2 * warp)) & 3u);
             const double *pb = reinterpret_cast<const double *>(sp + b0);
 
-            // store offsets of the outputs this step completes (plane t - 4), staged by the producer; -1: none
-            uint32_t io[16];
+            // store offsets of the outputs this step completes (plane t - N), staged by the producer; -1: none
+            uint32_t io[PY * PZ];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < PY; ++j) {
                 const uint4 q = *reinterpret_cast<const uint4 *>(sp + irow + j * 64);
                 io[4 * j] = q.x, io[4 * j + 1] = q.y, io[4 * j + 2] = q.z, io[4 * j + 3] = q.w;
             }
 
             if (mode == MODE_FULL) {
-                double ctr[4][4];
+                double ctr[PY][PZ];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    uint32_t pw[32];   // centre values of planes t-1 .. t-4 of this patch row
-                    if (!(SW_EXP & 2)) tm_ld32(t_in + j * 32, pw);
+                for (int j = 0; j < PY; ++j) {
+                    uint32_t pw[N * 8];   // centre values of planes t-1 .. t-N of this patch row
+                    if (!(SW_EXP & 2)) tm_ld_row<N>(t_in + j * S::ROW_WORDS, pw);
                     else
 #pragma unroll
-                        for (int q = 0; q < 32; ++q) pw[q] = io[q & 15] + q;
-                    double v[4 + 2 * N];
+                        for (int q = 0; q < N * 8; ++q) pw[q] = io[q & 7] + q;
+                    double v[PZ + 2 * N];
 #pragma unroll
-                    for (int tt = 0; tt < 4 + 2 * N; ++tt) v[tt] = (SW_EXP & 4) ? (tt == N ? pb[(j * SW_W + tt) * SW_C] : (double)(tt + j) * w0x3) : pb[(j * SW_W + tt) * SW_C];
+                    for (int tt = 0; tt < PZ + 2 * N; ++tt)
+                        v[tt] = (SW_EXP & 4) ? (tt == N ? pb[(j * WZ + tt) * SW_C] : (double)(tt + j) * w.w[1]) : pb[(j * WZ + tt) * SW_C];
                     const double2 va = *reinterpret_cast<const double2 *>(sp + vrow + j * 128);
                     const double2 vb = *reinterpret_cast<const double2 *>(sp + vrow + j * 128 + 16);
                     const double vv[4] = {va.x, va.y, vb.x, vb.y};
-                    double s[4];
+                    double s[PZ];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
+                    for (int i = 0; i < PZ; ++i) {
                         const double ce = v[N + i];
                         ctr[j][i] = ce;
 #pragma unroll
@@ -439,9 +497,9 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                         }
                     }
                     // backward half of the x arm from tensor memory, then park this row's centre values
-                    if (!(SW_EXP & 2)) tm_wait_ld32(pw);
+                    if (!(SW_EXP & 2)) tm_wait_row<N>(pw);
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
+                    for (int i = 0; i < PZ; ++i) {
 #pragma unroll
                         for (int k = 1; k <= N; ++k) {
                             const int sl = (PH + N - k) % N;
@@ -451,21 +509,22 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                     }
                     uint32_t cw[8];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
+                    for (int i = 0; i < PZ; ++i) {
                         cw[2 * i] = (uint32_t)__double2loint(ctr[j][i]);
                         cw[2 * i + 1] = (uint32_t)__double2hiint(ctr[j][i]);
                     }
-                    if (!(SW_EXP & 2)) tm_st8(t_in + j * 32 + PH * 8, cw);
+                    if (!(SW_EXP & 2)) tm_st8(t_in + j * S::ROW_WORDS + PH * 8, cw);
                 }
-                // y arms: rows 4py-4 .. 4py+7 of the patch's 4 z columns
+                // y arms: rows ty0-N .. ty0+PY-1+N of the patch's 4 z columns
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    double u[4 + 2 * N];
+                for (int i = 0; i < PZ; ++i) {
+                    double u[PY + 2 * N];
 #pragma unroll
-                    for (int tt = 0; tt < 4 + 2 * N; ++tt)
-                        u[tt] = (tt >= N && tt < N + 4) ? ctr[tt - N][i] : ((SW_EXP & 4) ? (double)(tt + i) * w0x3 : pb[((tt - N) * SW_W + N + i) * SW_C]);
+                    for (int tt = 0; tt < PY + 2 * N; ++tt)
+                        u[tt] = (tt >= N && tt < N + PY) ? ctr[tt - N][i]
+                                                         : ((SW_EXP & 4) ? (double)(tt + i) * w.w[1] : pb[((tt - N) * WZ + N + i) * SW_C]);
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
+                    for (int j = 0; j < PY; ++j)
 #pragma unroll
                         for (int k = 1; k <= N; ++k) {
                             acc[PH][j][i] = fma(w.w[k], u[N + j + k], acc[PH][j][i]);
@@ -475,11 +534,11 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             } else if (mode == MODE_CENTRE) {
                 // centre-only plane (warm-up / tail of a work item): it feeds the x arms of its neighbours
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < PY; ++j) {
                     uint32_t cw[8];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const double ce = pb[(j * SW_W + N + i) * SW_C];
+                    for (int i = 0; i < PZ; ++i) {
+                        const double ce = pb[(j * WZ + N + i) * SW_C];
 #pragma unroll
                         for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
                         const double out = fma(w.w[N], ce, acc[PH][j][i]);
@@ -488,7 +547,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                         cw[2 * i] = (uint32_t)__double2loint(ce);
                         cw[2 * i + 1] = (uint32_t)__double2hiint(ce);
                     }
-                    tm_st8(t_in + j * 32 + PH * 8, cw);
+                    tm_st8(t_in + j * S::ROW_WORDS + PH * 8, cw);
                 }
             } else {
                 // no mesh point of this warp's region in plane t: all centre values are zero
@@ -496,13 +555,13 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
 #pragma unroll
                 for (int q = 0; q < 8; ++q) cw[q] = 0u;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < PY; ++j) {
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
+                    for (int i = 0; i < PZ; ++i) {
                         store_if_valid(hp, io[4 * j + i], acc[PH][j][i]);
                         acc[PH][j][i] = 0.0;
                     }
-                    tm_st8(t_in + j * 32 + PH * 8, cw);
+                    tm_st8(t_in + j * S::ROW_WORDS + PH * 8, cw);
                 }
             }
             // this warp has read everything it needs from the stage
@@ -518,8 +577,19 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
     tm_wait_st();
 }
 
-template <bool TENSOR>
-__global__ void __launch_bounds__(SW_THREADS, 1)
+template <int REGS>
+__device__ __forceinline__ void setmaxnreg_inc()
+{
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(REGS));
+}
+template <int REGS>
+__device__ __forceinline__ void setmaxnreg_dec()
+{
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(REGS));
+}
+
+template <class S, bool TENSOR>
+__global__ void __launch_bounds__(S::THREADS, 1)
 sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_weights w, const __grid_constant__ sweep_maps maps)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -528,9 +598,9 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     __shared__ uint64_t rec_bar[SW_RING];
     __shared__ uint32_t tmem_base_s;
 
-    // threads 0..255: the 8 producer warps; threads 256..511: the 8 consumer warps (the higher warp ids, which the
-    // warp scheduler favours when several warps are ready)
-    const int tid = threadIdx.x, ctid = tid - (SW_THREADS - SW_CONSUMERS), warp = tid >> 5;
+    // threads 0..PRODUCERS-1: the producer warps; then the consumer warps (the higher warp ids, which the warp
+    // scheduler favours when several warps are ready)
+    const int tid = threadIdx.x, ctid = tid - S::PRODUCERS, warp = tid >> 5;
     const int2 item = a.items[blockIdx.x];
     const int nsteps = item.y;
     const long long clock0 = clock64();
@@ -539,13 +609,13 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
 #pragma unroll
         for (int s = 0; s < SW_STAGES; ++s) {
             mbar_init(smem_u32(&full_bar[s]), 4);   // the 4 warps of the producer group that stages the step
-            mbar_init(smem_u32(&empty_bar[s]), SW_CONSUMERS / 32);
+            mbar_init(smem_u32(&empty_bar[s]), S::NCW);
         }
 #pragma unroll
         for (int s = 0; s < SW_RING; ++s) mbar_init(smem_u32(&rec_bar[s]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    if (warp == (SW_THREADS - SW_CONSUMERS) / 32) {   // first consumer warp
+    if (warp == S::PRODUCERS / 32) {   // first consumer warp
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_base_s)),
                      "n"(SW_TMEM_COLS)
                      : "memory");
@@ -555,16 +625,17 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
 
-    // register re-split: 512 x 128 at launch = 256 x 32 (producers) + 256 x 224 (consumers); the pool that
-    // setmaxnreg.inc draws from holds only what setmaxnreg.dec released, so the two must balance exactly
+    // register re-split: THREADS x LAUNCH_REGS at launch -> PRODUCERS x PROD_REGS + CONSUMERS x CONS_REGS; the pool that
+    // setmaxnreg.inc draws from holds only what setmaxnreg.dec released, so the increase must not exceed the release
+    static_assert(S::CONSUMERS * (S::CONS_REGS - S::LAUNCH_REGS) <= S::PRODUCERS * (S::LAUNCH_REGS - S::PROD_REGS), "register pool");
     if (ctid < 0) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 32;\n");
-        sweep_producer<TENSOR>(a, maps, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), smem_u32(&rec_bar[0]),
-                               a.recs + (size_t)item.x * SW_REC_BYTES, nsteps, tid, 3.0 * w.w[0]);
+        setmaxnreg_dec<S::PROD_REGS>();
+        sweep_producer<S, TENSOR>(a, maps, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), smem_u32(&rec_bar[0]),
+                                  a.recs + (size_t)item.x * S::REC_BYTES, nsteps, tid, 3.0 * w.w[0]);
     } else {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;\n");
-        sweep_consumer(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid);
-        named_bar_sync(1, SW_CONSUMERS);
+        setmaxnreg_inc<S::CONS_REGS>();
+        sweep_consumer<S>(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid);
+        named_bar_sync(1, S::CONSUMERS);
         if (ctid == 0 && a.cycles) a.cycles[blockIdx.x] = clock64() - clock0;
         if (ctid < 32)
             asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base_s), "n"(SW_TMEM_COLS) : "memory");
@@ -579,9 +650,25 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
 static int g_max_planes = 32;   // x-slab thickness of a work item (rs_set_tuning("sweep_planes", v))
 static int g_force_tensor = 0;  // rs_set_tuning("sweep_tensor", 1): use the tensor-map copies also for 16 columns (tests)
 static int g_nctas = 0;         // rs_set_tuning("sweep_ctas", v): persistent CTAs (0 = one per SM)
+static int g_shape = 0;         // rs_set_tuning("sweep_shape", 1): fd_order 4 on the 12-warp shape (experiment)
 void rs_sweep_set_max_planes(int v) { g_max_planes = v < 4 ? 4 : v; }
 void rs_sweep_set_force_tensor(int v) { g_force_tensor = v != 0; }
 void rs_sweep_set_nctas(int v) { g_nctas = v < 0 ? 0 : v; }
+void rs_sweep_set_shape(int v) { g_shape = v; }
+
+namespace {
+enum { VARIANT_N4 = 0, VARIANT_N6 = 1, VARIANT_N4W12 = 2, VARIANT_NONE = -1 };
+int sweep_variant(int n)
+{
+    if (n == 4) return g_shape == 1 ? VARIANT_N4W12 : VARIANT_N4;
+    if (n == 6) return VARIANT_N6;
+    return VARIANT_NONE;
+}
+shape_rt variant_shape(int variant)
+{
+    return variant == VARIANT_N6 ? shape_of<shape_n6>() : variant == VARIANT_N4W12 ? shape_of<shape_n4w12>() : shape_of<shape_n4>();
+}
+}  // namespace
 
 namespace {
 
@@ -595,32 +682,34 @@ constexpr double COST_EMPTY_STEP = COST_STEP_FIXED;
 
 struct tile_geometry {
     const rs_mesh *m;
+    shape_rt sh;
     int nx, ny, nz, nty, ntz;
     int32_t point(int x, int y, int z) const
     {
         if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) return -1;
         return m->dense2point[rs_dense_index(m, x, y, z)];
     }
-    // 2 bits per warp for plane x of tile (iy, iz): which warps' 4 x 8 regions hold a mesh point
+    // 2 bits per warp for plane x of tile (iy, iz): which warps' PY x 8 regions hold a mesh point
+    // (a warp = two patches next to each other in z: patch rows PY * (w / 2) .., z columns 8 * (w % 2) ..)
     uint32_t warp_modes(int iy, int iz, int x, int mode) const
     {
         uint32_t hdr = 0;
-        for (int wq = 0; wq < 8; ++wq) {
+        for (int wq = 0; wq < sh.NCW; ++wq) {
             bool any = false;
-            for (int y = 4 * (wq >> 1); y < 4 * (wq >> 1) + 4 && !any; ++y)
-                for (int z = 8 * (wq & 1); z < 8 * (wq & 1) + 8 && !any; ++z) any = point(x, iy * SW_T + y, iz * SW_T + z) >= 0;
+            for (int y = sh.PY * (wq >> 1); y < sh.PY * (wq >> 1) + sh.PY && !any; ++y)
+                for (int z = 8 * (wq & 1); z < 8 * (wq & 1) + 8 && !any; ++z) any = point(x, iy * sh.TY + y, iz * SW_TZ + z) >= 0;
             if (any) hdr |= (uint32_t)mode << (2 * wq);
         }
         return hdr;
     }
 };
 
-double step_cost(uint32_t modes)
+double step_cost(uint32_t modes, int ncw)
 {
     double c = COST_STEP_FIXED;
-    for (int q = 0; q < 8; ++q) {
+    for (int q = 0; q < ncw; ++q) {
         const uint32_t md = (modes >> (2 * q)) & 3u;
-        c += md == MODE_FULL ? COST_FULL_WARP : md == MODE_CENTRE ? COST_CENTRE_WARP : 0.0;
+        c += (md == MODE_FULL ? COST_FULL_WARP : md == MODE_CENTRE ? COST_CENTRE_WARP : 0.0) * 8.0 / ncw;
     }
     return c;
 }
@@ -629,9 +718,12 @@ double step_cost(uint32_t modes)
 
 bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out)
 {
-    if (n != SW_N || ncol % SW_C != 0 || nctas < 1) return false;
-    const int N = SW_N, T = SW_T, W = SW_W;
-    tile_geometry g{m, m->dims[0], m->dims[1], m->dims[2], (m->dims[1] + T - 1) / T, (m->dims[2] + T - 1) / T};
+    const int variant = sweep_variant(n);
+    if (variant == VARIANT_NONE || ncol % SW_C != 0 || nctas < 1) return false;
+    const shape_rt sh = variant_shape(variant);
+    const int N = sh.N, TY = sh.TY, TZ = SW_TZ, WY = sh.WY, WZ = sh.WZ;
+    tile_geometry g{m, sh, m->dims[0], m->dims[1], m->dims[2], (m->dims[1] + TY - 1) / TY, (m->dims[2] + TZ - 1) / TZ};
+    out.rec_bytes = sh.rec_bytes;
     const int nx = g.nx, nchunks = ncol / SW_C;
     out = rs_sweep_host();
 
@@ -642,8 +734,8 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
             for (int x = 0; x < nx; ++x) {
                 const uint32_t mf = g.warp_modes(iy, iz, x, MODE_FULL);
                 if (mf) {
-                    fcost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(mf);
-                    ccost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(g.warp_modes(iy, iz, x, MODE_CENTRE));
+                    fcost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(mf, sh.NCW);
+                    ccost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(g.warp_modes(iy, iz, x, MODE_CENTRE), sh.NCW);
                 }
             }
     auto halo_cost = [&](int iy, int iz, int xa, int xb) {   // the 2 N centre-only steps around [xa, xb) + the piece's own overhead
@@ -755,44 +847,44 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
 
     // ---- records: one per (CTA, step) ----------------------------------------------------------------
     enum { UNKNOWN = 0, ZERO = 1, DATA = 2 };
-    std::vector<uint8_t> state((size_t)SW_STAGES * W * W);
+    std::vector<uint8_t> state((size_t)SW_STAGES * WY * WZ);
     out.items.resize(nctas);
     for (int cta = 0; cta < nctas; ++cta) {
         std::fill(state.begin(), state.end(), (uint8_t)UNKNOWN);   // shared memory of a starting CTA is arbitrary
         const int64_t first = out.nrec;
         int step = 0;                                               // stage of a step = step mod SW_STAGES, as in the kernel
         for (const rs_sweep_piece &pc : out.pieces[cta]) {
-            const int y0 = pc.iy * T, z0 = pc.iz * T;
+            const int y0 = pc.iy * TY, z0 = pc.iz * TZ;
             const int nsteps = (pc.xb - pc.xa) + 2 * N;
             for (int s = 0; s < nsteps; ++s, ++step) {
                 const int p = pc.xa - N + s;
                 const bool full = s >= N && s < nsteps - N;
-                out.recs.resize((size_t)(out.nrec + 1) * SW_REC_BYTES, 0);
-                unsigned char *rec = out.recs.data() + (size_t)out.nrec * SW_REC_BYTES;
+                out.recs.resize((size_t)(out.nrec + 1) * sh.rec_bytes, 0);
+                unsigned char *rec = out.recs.data() + (size_t)out.nrec * sh.rec_bytes;
                 uint2 *runs = reinterpret_cast<uint2 *>(rec + SW_REC_RUNS);
                 uint32_t *fill = reinterpret_cast<uint32_t *>(rec + SW_REC_FILL);
                 uint32_t *hdrp = reinterpret_cast<uint32_t *>(rec + SW_REC_HDR);
                 int32_t *cidx = reinterpret_cast<int32_t *>(rec + SW_REC_CIDX);
-                uint8_t *st = &state[(size_t)(step % SW_STAGES) * W * W];
+                uint8_t *st = &state[(size_t)(step % SW_STAGES) * WY * WZ];
                 // copy runs, and zero-fill bits for the slots this plane reads that are outside the mesh and
                 // do not already hold zeros from an earlier plane staged in the same buffer
                 int nrun = 0;
                 uint32_t tx1 = 0, tx2 = 0;
-                for (int r = full ? 0 : N; r < (full ? W : N + T); ++r) {
-                    const bool halo_row = r < N || r >= N + T;
-                    const int zlo = (halo_row || !full) ? N : 0, zhi = (halo_row || !full) ? N + T : W;
+                for (int r = full ? 0 : N; r < (full ? WY : N + TY); ++r) {
+                    const bool halo_row = r < N || r >= N + TY;
+                    const int zlo = (halo_row || !full) ? N : 0, zhi = (halo_row || !full) ? N + TZ : WZ;
                     int run_start = -1;
                     for (int zp = zlo; zp <= zhi; ++zp) {
                         const int32_t idx = zp < zhi ? g.point(p, y0 - N + r, z0 - N + zp) : -1;
                         if (idx >= 0) {
                             if (run_start < 0) run_start = zp;
-                            st[r * W + zp] = DATA;
+                            st[r * WZ + zp] = DATA;
                         } else {
                             if (run_start >= 0) {
                                 if (nrun >= SW_MAXRUN) return false;
                                 const int32_t firstp = g.point(p, y0 - N + r, z0 - N + run_start);
                                 const uint32_t len = (uint32_t)(zp - run_start);
-                                runs[nrun++] = make_uint2((uint32_t)firstp, (uint32_t)(r * W + run_start) | (len << 16));
+                                runs[nrun++] = make_uint2((uint32_t)firstp, (uint32_t)(r * WZ + run_start) | (len << 16));
                                 uint32_t box = 24;
                                 if (len < 24)
                                     for (box = 1; box * 2 <= len; box *= 2) {}
@@ -800,9 +892,9 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                                 tx2 += (box < len ? 2 * box : box) * SW_SLOT_BYTES;
                                 run_start = -1;
                             }
-                            if (zp < zhi && st[r * W + zp] != ZERO) {
-                                fill[(r * W + zp) >> 5] |= 1u << ((r * W + zp) & 31);
-                                st[r * W + zp] = ZERO;
+                            if (zp < zhi && st[r * WZ + zp] != ZERO) {
+                                fill[(r * WZ + zp) >> 5] |= 1u << ((r * WZ + zp) & 31);
+                                st[r * WZ + zp] = ZERO;
                             }
                         }
                     }
@@ -811,8 +903,8 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                 hdrp[1] = (uint32_t)(pc.chunk * SW_C);
                 hdrp[2] = tx1;
                 hdrp[3] = tx2;
-                for (int y = 0; y < T; ++y)
-                    for (int z = 0; z < T; ++z) cidx[y * T + z] = full ? g.point(p, y0 + y, z0 + z) : -1;
+                for (int y = 0; y < TY; ++y)
+                    for (int z = 0; z < TZ; ++z) cidx[y * TZ + z] = full ? g.point(p, y0 + y, z0 + z) : -1;
                 ++out.nrec;
             }
         }
@@ -823,15 +915,32 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
 
 bool rs_sweep_supported(const rs_mesh *m, int n, int ncol)
 {
-    return m->ordering == RS_ORDER_LEX && !m->periodic && n == SW_N && ncol >= SW_C && ncol % SW_C == 0 &&
+    return m->ordering == RS_ORDER_LEX && !m->periodic && sweep_variant(n) != VARIANT_NONE && ncol >= SW_C && ncol % SW_C == 0 &&
            (uint64_t)(m->np + 1) * (uint64_t)ncol < 0xffffffffull;   // store offsets are 32-bit element offsets
 }
 
 static int sweep_nctas(const rs_mesh *m) { return g_nctas > 0 ? g_nctas : (m->sm_count > 0 ? m->sm_count : 148); }
 
+template <class S>
+static cudaError_t set_smem()
+{
+    cudaError_t e = cudaFuncSetAttribute(sweep_kernel<S, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(sweep_kernel<S, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
+}
+
+template <class S>
+static void launch_shape(bool tensor, unsigned grid, cudaStream_t st, const sweep_args &a, const rs_weights &w, const sweep_maps &maps)
+{
+    if (tensor)
+        sweep_kernel<S, true><<<grid, S::THREADS, S::SMEM, st>>>(a, w, maps);
+    else
+        sweep_kernel<S, false><<<grid, S::THREADS, S::SMEM, st>>>(a, w, maps);
+}
+
 static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables **out)
 {
-    const auto key = std::make_pair(n, ncol);
+    const auto key = std::make_pair(n * 16 + sweep_variant(n), ncol);
     auto f = m->sweep.find(key);
     if (f == m->sweep.end()) {
         rs_sweep_host h;
@@ -850,16 +959,18 @@ static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables *
             RS_CUDA_TRY(up((void **)&tb.d_recs, h.recs.data(), h.recs.size()));
             RS_CUDA_TRY(cudaMalloc((void **)&tb.d_cycles, (h.items.size() + 2048) * sizeof(long long)));
             RS_CUDA_TRY(cudaMemset(tb.d_cycles, 0, (h.items.size() + 2048) * sizeof(long long)));
+            tb.variant = sweep_variant(n);
             for (size_t c = 0; c < h.items.size(); ++c) {
                 int64_t nfull = 0;
                 for (int t = 0; t < h.items[c].y; ++t) {
-                    const uint32_t hd = *reinterpret_cast<const uint32_t *>(h.recs.data() + (size_t)(h.items[c].x + t) * SW_REC_BYTES + SW_REC_HDR);
-                    for (int wq = 0; wq < 8; ++wq) nfull += ((hd >> (2 * wq)) & 3u) == MODE_FULL;
+                    const uint32_t hd = *reinterpret_cast<const uint32_t *>(h.recs.data() + (size_t)(h.items[c].x + t) * h.rec_bytes + SW_REC_HDR);
+                    for (int wq = 0; wq < 12; ++wq) nfull += ((hd >> (2 * wq)) & 3u) == MODE_FULL;
                 }
                 tb.host_stats.insert(tb.host_stats.end(), {(int64_t)h.items[c].y, (int64_t)h.pieces[c].size(), (int64_t)(h.load[c] * 1000), nfull});
             }
-            RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
-            RS_CUDA_TRY(cudaFuncSetAttribute(sweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SW_SMEM));
+            RS_CUDA_TRY(set_smem<shape_n4>());
+            RS_CUDA_TRY(set_smem<shape_n6>());
+            RS_CUDA_TRY(set_smem<shape_n4w12>());
         }
         f = m->sweep.emplace(key, tb).first;
     }
@@ -914,11 +1025,16 @@ rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const d
         if (((uintptr_t)psi & 15u) != 0) return rs_fail(RS_ERR_INVALID_ARG, "psi must be 16-byte aligned");
         rc = encode_maps(m, psi, ncol, maps);
         if (rc != RS_OK) return rc;
-        sweep_kernel<true><<<(unsigned)tb->nitems, SW_THREADS, SW_SMEM, st>>>(a, w, maps);
     } else {
         std::memset(&maps, 0, sizeof(maps));
-        sweep_kernel<false><<<(unsigned)tb->nitems, SW_THREADS, SW_SMEM, st>>>(a, w, maps);
     }
+    const unsigned grid = (unsigned)tb->nitems;
+    if (tb->variant == VARIANT_N6)
+        launch_shape<shape_n6>(tensor, grid, st, a, w, maps);
+    else if (tb->variant == VARIANT_N4W12)
+        launch_shape<shape_n4w12>(tensor, grid, st, a, w, maps);
+    else
+        launch_shape<shape_n4>(tensor, grid, st, a, w, maps);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
 }
@@ -936,17 +1052,21 @@ int64_t rs_sweep_table_bytes(const rs_mesh *cm, int n, int ncol)
 {
     rs_mesh *m = const_cast<rs_mesh *>(cm);
     if (!rs_sweep_supported(m, n, ncol)) return 0;
-    auto f = m->sweep.find(std::make_pair(n, ncol));
+    auto f = m->sweep.find(std::make_pair(n * 16 + sweep_variant(n), ncol));
     if (f != m->sweep.end()) return f->second.bytes;
     rs_sweep_host h;   // no device (or not built yet): count on the host
     if (!rs_sweep_build_host(m, n, ncol, g_max_planes, sweep_nctas(m), h)) return 0;
     return (int64_t)(h.items.size() * sizeof(int2) + h.recs.size());
 }
 
-const char *rs_sweep_variant_name(const rs_mesh *, int, int ncol)
+const char *rs_sweep_variant_name(const rs_mesh *, int n, int ncol)
 {
-    return (ncol != SW_C || g_force_tensor) ? "sweep[n4 c16 16x16 q4p4 persistent ws tma2d+tmem s3]"
-                                            : "sweep[n4 c16 16x16 q4p4 persistent ws tma1d+tmem s3]";
+    const bool tensor = ncol != SW_C || g_force_tensor;
+    switch (sweep_variant(n)) {
+        case VARIANT_N6: return tensor ? "sweep[n6 c16 8x16 q2p4 persistent ws tma2d+tmem s3]" : "sweep[n6 c16 8x16 q2p4 persistent ws tma1d+tmem s3]";
+        case VARIANT_N4W12: return tensor ? "sweep[n4 c16 12x16 q2p4 persistent ws tma2d+tmem s3]" : "sweep[n4 c16 12x16 q2p4 persistent ws tma1d+tmem s3]";
+        default: return tensor ? "sweep[n4 c16 16x16 q4p4 persistent ws tma2d+tmem s3]" : "sweep[n4 c16 16x16 q4p4 persistent ws tma1d+tmem s3]";
+    }
 }
 
 void rs_sweep_free(rs_mesh *m)
@@ -969,7 +1089,8 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
     if (!rs_sweep_supported(m, n, ncol)) return "unsupported (ordering / order / width)";
     rs_sweep_host h;
     if (!rs_sweep_build_host(m, n, ncol, max_planes, nctas, h)) return "a plane needs more copy runs than a record holds";
-    const int N = SW_N, T = SW_T, W = SW_W, NS = 6 * N;
+    const shape_rt sh = variant_shape(sweep_variant(n));
+    const int N = sh.N, TY = sh.TY, TZ = SW_TZ, WY = sh.WY, WZ = sh.WZ, NS = 6 * N;
     const int64_t np = m->np;
     std::vector<int32_t> map((size_t)np * NS);
     rs_build_index_map(m, n, map.data());
@@ -987,38 +1108,38 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
     const int32_t UNK = -2;
     for (int cta = 0; cta < nctas; ++cta) {
         npieces += (int64_t)h.pieces[cta].size();
-        std::vector<int32_t> stage((size_t)SW_STAGES * W * W, UNK);
+        std::vector<int32_t> stage((size_t)SW_STAGES * WY * WZ, UNK);
         // per tile point: centre values seen at the last 4 steps and the outputs pending from them
-        std::vector<int32_t> hist((size_t)T * T * N, UNK), pend((size_t)T * T * N, -1), pend_chunk((size_t)T * T * N, 0);
+        std::vector<int32_t> hist((size_t)TY * TZ * N, UNK), pend((size_t)TY * TZ * N, -1), pend_chunk((size_t)TY * TZ * N, 0);
         const int nsteps = h.items[cta].y;
         for (int t = 0; t < nsteps; ++t) {
-            const unsigned char *rec = h.recs.data() + (size_t)(h.items[cta].x + t) * SW_REC_BYTES;
+            const unsigned char *rec = h.recs.data() + (size_t)(h.items[cta].x + t) * sh.rec_bytes;
             const uint2 *runs = reinterpret_cast<const uint2 *>(rec + SW_REC_RUNS);
             const uint32_t *fill = reinterpret_cast<const uint32_t *>(rec + SW_REC_FILL);
             const uint32_t *hdr = reinterpret_cast<const uint32_t *>(rec + SW_REC_HDR);
             const int32_t *cidx = reinterpret_cast<const int32_t *>(rec + SW_REC_CIDX);
-            int32_t *sg = &stage[(size_t)(t % SW_STAGES) * W * W];
+            int32_t *sg = &stage[(size_t)(t % SW_STAGES) * WY * WZ];
             uint32_t tx1 = 0;
             for (int r = 0; r < SW_MAXRUN; ++r) {
                 const uint32_t len = runs[r].y >> 16, slot = runs[r].y & 0xffffu;
-                if (slot + len > (uint32_t)(W * W)) return fail(cta, t, "run leaves the stage", 0, 0, r);
+                if (slot + len > (uint32_t)(WY * WZ)) return fail(cta, t, "run leaves the stage", 0, 0, r);
                 for (uint32_t i = 0; i < len; ++i) sg[slot + i] = (int32_t)(runs[r].x + i);
                 tx1 += len * SW_SLOT_BYTES;
             }
             if (tx1 != hdr[2]) return fail(cta, t, "byte count of the copy runs", 0, 0, 0);
-            for (int r = 0; r < W; ++r)
-                for (int z = 0; z < W; ++z)
-                    if ((fill[(r * W + z) >> 5] >> ((r * W + z) & 31)) & 1u) sg[r * W + z] = -1;
+            for (int r = 0; r < WY; ++r)
+                for (int z = 0; z < WZ; ++z)
+                    if ((fill[(r * WZ + z) >> 5] >> ((r * WZ + z) & 31)) & 1u) sg[r * WZ + z] = -1;
             const int chunk = (int)hdr[1] / SW_C;
             const int ph = t % N;
-            for (int y = 0; y < T; ++y)
-                for (int z = 0; z < T; ++z) {
-                    const int wq = (y / 4) * 2 + z / 8;
+            for (int y = 0; y < TY; ++y)
+                for (int z = 0; z < TZ; ++z) {
+                    const int wq = (y / sh.PY) * 2 + z / 8;
                     const int mode = (int)((hdr[0] >> (2 * wq)) & 3u);
-                    const int32_t ci = (hdr[0] & HDR_OUTPUT_PLANE) ? cidx[y * T + z] : -1;
-                    int32_t *hp = &hist[(size_t)(y * T + z) * N], *pp = &pend[(size_t)(y * T + z) * N];
-                    int32_t *pc = &pend_chunk[(size_t)(y * T + z) * N];
-                    const int32_t ce = mode == MODE_EMPTY ? -1 : sg[(N + y) * W + N + z];
+                    const int32_t ci = (hdr[0] & HDR_OUTPUT_PLANE) ? cidx[y * TZ + z] : -1;
+                    int32_t *hp = &hist[(size_t)(y * TZ + z) * N], *pp = &pend[(size_t)(y * TZ + z) * N];
+                    int32_t *pc = &pend_chunk[(size_t)(y * TZ + z) * N];
+                    const int32_t ce = mode == MODE_EMPTY ? -1 : sg[(N + y) * WZ + N + z];
                     // forward half of the x arm of the outputs pending from the last 4 steps
                     for (int k = 1; k <= N; ++k) {
                         const int32_t o = pp[(ph + N - k) % N];
@@ -1038,10 +1159,10 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
                         if (mode != MODE_FULL) return fail(cta, t, "output point in a warp that skips the plane", y, z, 0);
                         if (ce != ci) return fail(cta, t, "centre value", y, z, 0);
                         for (int k = 1; k <= N; ++k) {
-                            if (sg[(N + y) * W + N + z + k] != arm(ci, 2, k)) return fail(cta, t, "z arm", y, z, k);
-                            if (sg[(N + y) * W + N + z - k] != arm(ci, 2, -k)) return fail(cta, t, "z arm", y, z, -k);
-                            if (sg[(N + y + k) * W + N + z] != arm(ci, 1, k)) return fail(cta, t, "y arm", y, z, k);
-                            if (sg[(N + y - k) * W + N + z] != arm(ci, 1, -k)) return fail(cta, t, "y arm", y, z, -k);
+                            if (sg[(N + y) * WZ + N + z + k] != arm(ci, 2, k)) return fail(cta, t, "z arm", y, z, k);
+                            if (sg[(N + y) * WZ + N + z - k] != arm(ci, 2, -k)) return fail(cta, t, "z arm", y, z, -k);
+                            if (sg[(N + y + k) * WZ + N + z] != arm(ci, 1, k)) return fail(cta, t, "y arm", y, z, k);
+                            if (sg[(N + y - k) * WZ + N + z] != arm(ci, 1, -k)) return fail(cta, t, "y arm", y, z, -k);
                             if (hp[(ph + N - k) % N] != arm(ci, 0, -k)) return fail(cta, t, "backward x arm", y, z, -k);
                         }
                     }
@@ -1067,7 +1188,7 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
 int64_t rs_sweep_read_stats(const rs_mesh *cm, int n, int ncol, int64_t *out, int64_t max_ctas)
 {
     rs_mesh *m = const_cast<rs_mesh *>(cm);
-    auto f = m->sweep.find(std::make_pair(n, ncol));
+    auto f = m->sweep.find(std::make_pair(n * 16 + sweep_variant(n), ncol));
     if (f == m->sweep.end() || !f->second.ok) return 0;
     const rs_sweep_tables &t = f->second;
     const int64_t nc = std::min<int64_t>(t.nitems, max_ctas);

@@ -97,6 +97,37 @@ def test_sweep_kernel_variants(knob):
     check(g, o, problem(1).cond_denominator(psi, 4), f"sweep variant {knob}")
 
 
+@pytest.mark.parametrize("B,is_complex", [(16, False), (64, False), (8, True)])
+def test_sweep_kernel_order6(B, is_complex):
+    """fd_order 6 through the plane-sweep kernel's 8 x 16 / 2 x 4 shape (config 1 mesh; ragged last block)."""
+    key = ("c1n6",)
+    if key not in _cache:
+        cfg = synthetic.config(1)
+        _cache[key] = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=6)
+    p = _cache[key]
+    psi = synthetic.orbitals(61, 0, B + 3, p.np, is_complex=is_complex)
+    g = _run(p, psi, 6, B, "sweep")
+    assert rs.rs_kernel_name(p.mesh, 6, B, rs.RS_COMPLEX128 if is_complex else rs.RS_REAL64, rs.RS_KERNEL_SWEEP).startswith("sweep[n6")
+    o = p.oracle_hpsi(psi, 6)
+    check(g, o, p.cond_denominator(psi, 6), f"sweep n=6 B={B}")
+
+
+@pytest.mark.parametrize("B", [16, 32])
+def test_sweep_kernel_12_warp_shape(B):
+    """fd_order 4 on the experimental 12 x 16 / 2 x 4 shape with 12 consumer warps."""
+    cfg = synthetic.config(1)
+    rs.rs_set_tuning("sweep_shape", 1)
+    try:
+        p = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=4)
+        psi = synthetic.orbitals(cfg.seed, 0, B + 1, p.np)
+        g = p.gpu_hpsi(psi, 4, B, kernel=rs.RS_KERNEL_SWEEP)
+        assert rs.rs_kernel_name(p.mesh, 4, B, kernel=rs.RS_KERNEL_SWEEP).startswith("sweep[n4 c16 12x16")
+    finally:
+        rs.rs_set_tuning("sweep_shape", 0)
+    o = problem(1).oracle_hpsi(psi, 4)
+    check(g, o, problem(1).cond_denominator(psi, 4), f"12-warp shape B={B}")
+
+
 def test_sweep_kernel_dirichlet_boxes():
     """Non-periodic boxes through the plane-sweep kernel: sizes that are not multiples of the 16 x 16 tile."""
     for box in [(24, 24, 24), (7, 9, 10), (1, 1, 37), (13, 1, 5), (40, 17, 33)]:

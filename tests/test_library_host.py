@@ -205,6 +205,19 @@ def test_sweep_records_expand_to_the_plain_table(cfg_i, nst, dtype, planes, ncta
     assert st["nctas"] == nctas and st["records"] > 0 and st["cost_max"] >= st["cost_mean"] > 0
 
 
+@pytest.mark.parametrize("cfg_i,n,nst,shape", [(0, 6, 16, 0), (1, 6, 16, 0), (1, 6, 64, 0), (1, 4, 16, 1), (1, 4, 32, 1)])
+def test_sweep_records_other_kernel_shapes(cfg_i, n, nst, shape):
+    """fd_order 6 (8 x 16 tiles, 2 x 4 patches) and the 12-warp shape for fd_order 4 (12 x 16 tiles)."""
+    cfg = synthetic.config(cfg_i)
+    mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, 6)
+    rs.rs_set_tuning("sweep_shape", shape)
+    try:
+        st = rs.rs_sweep_selfcheck(mesh, n, nst, rs.RS_REAL64, 32, 148)
+    finally:
+        rs.rs_set_tuning("sweep_shape", 0)
+    assert st["records"] > 0
+
+
 def test_sweep_selfcheck_on_boxes_and_unsupported_calls():
     for box in [(24, 24, 24), (7, 9, 10), (1, 1, 37), (40, 17, 33)]:
         mesh = rs.rs_mesh_create_box(*box, 0.25, 4, False, rs.RS_ORDER_LEX)
@@ -213,7 +226,10 @@ def test_sweep_selfcheck_on_boxes_and_unsupported_calls():
     with pytest.raises(rs.RsError) as e:
         rs.rs_sweep_selfcheck(mesh, 4, 16)
     assert e.value.status == rs.RS_ERR_UNSUPPORTED
-    mesh = rs.rs_mesh_create_box(8, 8, 8, 0.25, 4, False, rs.RS_ORDER_LEX)
+    mesh = rs.rs_mesh_create_box(8, 8, 8, 0.25, 5, False, rs.RS_ORDER_LEX)
     with pytest.raises(rs.RsError) as e:
         rs.rs_sweep_selfcheck(mesh, 4, 8)                                           # 8 real columns: gather kernel only
+    assert e.value.status == rs.RS_ERR_UNSUPPORTED
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_sweep_selfcheck(mesh, 5, 16)                                          # fd_order 5: gather kernel only
     assert e.value.status == rs.RS_ERR_UNSUPPORTED
