@@ -180,6 +180,7 @@ def main() -> None:
     ap.add_argument("--sweep", action="store_true", help="also time apply alone for every block size of the config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-autotune", action="store_true", help="skip rs_hamiltonian_autotune (work dealt by the built-in cost model)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
@@ -256,6 +257,12 @@ def main() -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
+    # once per geometry, like the mesh tables: let the library measure its own per-plane costs and re-deal the work
+    t = time.perf_counter()
+    if not args.no_autotune and args.kernel != "gather":
+        rs.rs_block_pack(mesh, states, 0, min(B, nst), B, blk)
+        rs.rs_hamiltonian_autotune(mesh, n, coeffs, v, blk, hblk, B)
+    t_tune = time.perf_counter() - t
     for _ in range(args.warmup):
         step(False)
     barrier()
@@ -308,6 +315,8 @@ def main() -> None:
             b2 = torch.empty((npts + 1, Bs), dtype=tdt, device=dev)
             rs.rs_block_pack(mesh, states, 0, min(Bs, nst), Bs, b1)
             reps = max(3, min(50, int(nst // Bs)))
+            if not args.no_autotune and args.kernel != "gather":
+                rs.rs_hamiltonian_autotune(mesh, n, coeffs, v, b1, b2, Bs)
             for _ in range(3):
                 rs.rs_hamiltonian_apply(mesh, n, coeffs, v, b1, b2, Bs, kernel=kern)
             torch.cuda.synchronize()
@@ -353,7 +362,7 @@ def main() -> None:
                 "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "c128" if is_c else "f64", "data": "synthetic",
                 "config": {**workload_config(cfg, n, B, npts), "kernel": kname, "parallelism": f"orbital-blocks x{world}",
-                           "mesh_build_s": t_mesh, "nbricks": mesh.nbricks},
+                           "mesh_build_s": t_mesh, "autotune_s": t_tune, "autotuned": not args.no_autotune, "nbricks": mesh.nbricks},
                 "roofline": roofline, "clocks": clocks, "gpu_launches": 3 * nblocks * args.steps}
         if e2e:
             line["e2e"] = e2e

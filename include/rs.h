@@ -130,6 +130,15 @@ rs_status rs_hamiltonian_apply_v(const rs_mesh *mesh, int fd_order, const double
                                  const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
                                  rs_dtype dtype, void *stream, rs_kernel kernel);
 
+/* Optional, once per (mesh, fd_order, nst, dtype): "measure, don't guess".  Runs the kernel a few times on the
+ * caller's buffers (arguments as rs_hamiltonian_apply; hpsi receives H psi), reads back the clock each persistent
+ * CTA recorded at the end of every plane, and deals the work to the CTAs again using the measured cost of every
+ * (tile, plane) instead of the built-in cost model.  Later rs_hamiltonian_apply calls use the re-dealt tables; results
+ * are unchanged up to rounding order.  SYNCHRONISES `stream`.  A call that the gather kernel serves is just applied. */
+rs_status rs_hamiltonian_autotune(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
+                                  const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
+                                  rs_dtype dtype, void *stream);
+
 /* ---- whole path on HOST buffers (step a7: the block sweep; used for the end-to-end number) --------
  * states_host / hstates_host: pinned or pageable host arrays [nst_total][ld] (ld >= np, mesh order);
  * vloc_host [np].  Uploads, then for each block of `block_size` orbitals: pack, apply, unpack; then

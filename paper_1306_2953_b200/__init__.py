@@ -36,7 +36,7 @@ EXPORTS = (
     "rs_mesh_spacing", "rs_mesh_nbricks", "rs_mesh_get_points", "rs_mesh_get_index_map", "rs_block_bytes",
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
     "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version", "rs_set_tuning",
-    "rs_sweep_selfcheck", "rs_sweep_stats",
+    "rs_sweep_selfcheck", "rs_sweep_stats", "rs_hamiltonian_autotune",
 )
 
 
@@ -72,6 +72,7 @@ def _load() -> C.CDLL:
     L.rs_block_pack.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, vp, C.c_int, vp]
     L.rs_block_unpack.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int64, C.c_int, C.c_int, vp]
     L.rs_hamiltonian_apply.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp]
+    L.rs_hamiltonian_autotune.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp]
     L.rs_hamiltonian_apply_v.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp, C.c_int]
     L.rs_hamiltonian_apply_states_host.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int]
     L.rs_last_error.restype = C.c_char_p
@@ -251,6 +252,18 @@ def rs_hamiltonian_apply(mesh: Mesh, fd_order: int, coeffs, vloc, psi, hpsi, nst
     dtype = _dtype_of(psi) if dtype is None else dtype
     _check(_lib.rs_hamiltonian_apply_v(mesh.handle, fd_order, _dptr(c), _ptr(vloc), _ptr(psi), _ptr(hpsi), nst,
                                        dtype, _stream(stream), kernel))
+
+
+def rs_hamiltonian_autotune(mesh: Mesh, fd_order: int, coeffs, vloc, psi, hpsi, nst: int, dtype: int | None = None,
+                            stream=None) -> None:
+    """Once per (mesh, order, width): measure the plane-sweep kernel's per-step costs on these buffers and re-deal the
+    work to the CTAs accordingly (synchronises the stream; hpsi receives H psi)."""
+    c = np.ascontiguousarray(coeffs, dtype=np.float64)
+    if c.shape != (fd_order + 1,):
+        raise RsError(RS_ERR_INVALID_ARG, "coeffs must hold c_0..c_n")
+    dtype = _dtype_of(psi) if dtype is None else dtype
+    _check(_lib.rs_hamiltonian_autotune(mesh.handle, fd_order, _dptr(c), _ptr(vloc), _ptr(psi), _ptr(hpsi), nst, dtype,
+                                        _stream(stream)))
 
 
 def rs_hamiltonian_apply_states_host(mesh: Mesh, fd_order: int, coeffs, vloc_host, states_host, hstates_host,

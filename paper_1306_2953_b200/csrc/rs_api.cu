@@ -72,6 +72,21 @@ extern "C" rs_status rs_hamiltonian_apply_v(const rs_mesh *m, int n, const doubl
     return rs_launch_gather(m, n, w, d_map, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
 }
 
+extern "C" rs_status rs_hamiltonian_autotune(const rs_mesh *m, int n, const double *coeffs, const double *vloc, const void *psi,
+                                             void *hpsi, int nst, rs_dtype dtype, void *stream)
+{
+    rs_status st = check_apply(m, n, coeffs, vloc, psi, hpsi, nst, dtype);
+    if (st != RS_OK) return st;
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    rs_weights w;
+    std::memset(&w, 0, sizeof(w));
+    for (int k = 0; k <= n; ++k) w.w[k] = -0.5 * coeffs[k] / (m->h * m->h);
+    const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
+    if (resolve_kernel(m, n, ncol, RS_KERNEL_AUTO) != RS_KERNEL_SWEEP)   // gather kernel: nothing to tune, just apply
+        return rs_hamiltonian_apply(m, n, coeffs, vloc, psi, hpsi, nst, dtype, stream);
+    return rs_sweep_autotune(m, n, w, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
+}
+
 extern "C" rs_status rs_hamiltonian_apply(const rs_mesh *m, int n, const double *coeffs, const double *vloc,
                                           const void *psi, void *hpsi, int nst, rs_dtype dtype, void *stream)
 {

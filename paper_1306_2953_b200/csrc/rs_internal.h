@@ -35,9 +35,16 @@ struct rs_sweep_host {
     std::vector<std::vector<rs_sweep_piece>> pieces; // per CTA, in execution order
     std::vector<unsigned char> recs;                 // [nrec][rec_bytes]
     int rec_bytes = 0;                               // 608 + 4 per tile point (depends on the kernel shape)
+    std::vector<int32_t> rec_cell;                   // per record: tile * nx + x of an output plane, -1 for a halo step
     int64_t nrec = 0;
     std::vector<double> load;                        // modelled load per CTA
     double cost_max = 0.0, cost_mean = 0.0;          // modelled load of the busiest / average CTA
+};
+// measured cost of the kernel's steps on this mesh (rs_hamiltonian_autotune): replaces the cost model when dealing
+struct rs_sweep_costs {
+    std::vector<float> full;      // [tiles * nx] mean clocks of an output step of (tile, plane); 0 = not measured
+    double halo = 0.0;            // mean clocks of a halo step
+    double unit = 0.0;            // mean clocks of an output step (all values are used relative to it)
 };
 struct rs_sweep_tables {
     bool ok = false;              // false: some plane needs more than RS_SWEEP_MAXRUN runs (use the gather kernel)
@@ -46,6 +53,9 @@ struct rs_sweep_tables {
     int2 *d_items = nullptr;
     unsigned char *d_recs = nullptr;
     long long *d_cycles = nullptr;                   // per CTA: clock ticks of the last launch
+    long long *d_step_clock = nullptr;               // per record: clock at the end of that step (last launch)
+    std::vector<int2> host_items;                    // copies kept for rs_hamiltonian_autotune
+    std::vector<int32_t> rec_cell;
     std::vector<int64_t> host_stats;                 // per CTA: {steps, pieces, modelled load x 1000, full warp-steps}
 };
 
@@ -70,6 +80,7 @@ struct rs_mesh {
     int sm_count = 0;
     int32_t *d_map[RS_MAX_FD_ORDER + 1] = {nullptr};                 // [np][6n], built lazily per order
     std::map<std::pair<int, int>, rs_sweep_tables> sweep;            // (fd_order, ncol) -> tables, built lazily
+    std::map<std::pair<int, int>, rs_sweep_costs> sweep_costs;       // measured step costs, if autotuned
 };
 
 void rs_set_error(const std::string &msg);
@@ -110,4 +121,7 @@ int64_t rs_sweep_table_bytes(const rs_mesh *m, int n, int ncol);
 const char *rs_sweep_variant_name(const rs_mesh *m, int n, int ncol);
 void rs_sweep_free(rs_mesh *m);
 // host-only construction of the records; false if a plane needs more than RS_SWEEP_MAXRUN runs
-bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out);
+bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out,
+                         const rs_sweep_costs *measured = nullptr);
+rs_status rs_sweep_autotune(const rs_mesh *m, int n, const rs_weights &w, const double *vloc, const double *psi, double *hpsi,
+                            int ncol, cudaStream_t st);

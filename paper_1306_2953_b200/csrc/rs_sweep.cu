@@ -228,6 +228,7 @@ struct sweep_args {
     double *hpsi;
     uint32_t ncol;               // row pitch of the block in elements
     long long *cycles;           // optional [gridDim.x]: clock64 ticks each CTA spent (calibration of the cost model)
+    long long *step_clock;       // optional [nrec]: clock64 at the end of every step (rs_hamiltonian_autotune)
 };
 struct sweep_maps {
     CUtensorMap box[SW_NBOX];    // psi as a [np+1][ncol] fp64 tensor, box {16, 1|2|4|8|16|24}
@@ -416,7 +417,8 @@ __device__ __forceinline__ void tm_wait_row(uint32_t (&r)[N * 8])
 
 template <class S>
 __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_weights &w, const unsigned char *smem,
-                                               uint32_t full0, uint32_t empty0, uint32_t tmem_base, int nsteps, int tid)
+                                               uint32_t full0, uint32_t empty0, uint32_t tmem_base, int nsteps, int tid,
+                                               long long *step_clock)
 {
     constexpr int N = S::N, PY = S::PY, PZ = SW_PZ, WZ = S::WZ;
     const int lane = tid & 31, warp = tid >> 5;
@@ -568,6 +570,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             __syncwarp();
             SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 6);
             if (lane == 0) mbar_arrive(empty0 + 8u * stage);
+            if (tid == 0 && step_clock) step_clock[t] = clock64();
             if (++stage == SW_STAGES) {
                 stage = 0;
                 parity ^= 1u;
@@ -634,7 +637,8 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
                                   a.recs + (size_t)item.x * S::REC_BYTES, nsteps, tid, 3.0 * w.w[0]);
     } else {
         setmaxnreg_inc<S::CONS_REGS>();
-        sweep_consumer<S>(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid);
+        sweep_consumer<S>(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid,
+                          a.step_clock ? a.step_clock + item.x : nullptr);
         named_bar_sync(1, S::CONSUMERS);
         if (ctid == 0 && a.cycles) a.cycles[blockIdx.x] = clock64() - clock0;
         if (ctid < 32)
@@ -716,7 +720,8 @@ double step_cost(uint32_t modes, int ncw)
 
 }  // namespace
 
-bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out)
+bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out,
+                         const rs_sweep_costs *measured)
 {
     const int variant = sweep_variant(n);
     if (variant == VARIANT_NONE || ncol % SW_C != 0 || nctas < 1) return false;
@@ -738,19 +743,34 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                     ccost[((size_t)iy * g.ntz + iz) * nx + x] = step_cost(g.warp_modes(iy, iz, x, MODE_CENTRE), sh.NCW);
                 }
             }
+    // measured step costs (rs_hamiltonian_autotune), relative to the mean output step, replace the model where present
+    double cost_piece = COST_PIECE, cost_empty = COST_EMPTY_STEP;
+    if (measured && measured->unit > 0.0 && measured->full.size() == fcost.size()) {
+        double ratio_sum = 0.0;   // measured / model over the measured cells: scales the model for the others
+        int64_t ratio_n = 0;
+        for (size_t q = 0; q < fcost.size(); ++q)
+            if (fcost[q] > 0.0 && measured->full[q] > 0.f) ratio_sum += measured->full[q] / measured->unit / fcost[q], ++ratio_n;
+        const double scale = ratio_n ? ratio_sum / ratio_n : 1.0;
+        for (size_t q = 0; q < fcost.size(); ++q)
+            if (fcost[q] > 0.0) fcost[q] = measured->full[q] > 0.f ? measured->full[q] / measured->unit : fcost[q] * scale;
+        cost_empty = measured->halo / measured->unit;
+        for (double &c : ccost)
+            if (c > 0.0) c = cost_empty;
+        cost_piece = 0.0;   // a piece's start-up is part of its measured steps
+    }
     auto halo_cost = [&](int iy, int iz, int xa, int xb) {   // the 2 N centre-only steps around [xa, xb) + the piece's own overhead
-        double c = COST_PIECE;
+        double c = cost_piece;
         const double *cc = &ccost[((size_t)iy * g.ntz + iz) * nx];
         for (int k = 1; k <= N; ++k) {
-            c += (xa - k >= 0 && cc[xa - k] > 0.0) ? cc[xa - k] : COST_EMPTY_STEP;
-            c += (xb + k - 1 < nx && cc[xb + k - 1] > 0.0) ? cc[xb + k - 1] : COST_EMPTY_STEP;
+            c += (xa - k >= 0 && cc[xa - k] > 0.0) ? cc[xa - k] : cost_empty;
+            c += (xb + k - 1 < nx && cc[xb + k - 1] > 0.0) ? cc[xb + k - 1] : cost_empty;
         }
         return c;
     };
     auto range_cost = [&](int iy, int iz, int xa, int xb) {
         double c = 0.0;
         const double *fc = &fcost[((size_t)iy * g.ntz + iz) * nx];
-        for (int x = xa; x < xb; ++x) c += fc[x] > 0.0 ? fc[x] : COST_EMPTY_STEP;
+        for (int x = xa; x < xb; ++x) c += fc[x] > 0.0 ? fc[x] : cost_empty;
         return c;
     };
 
@@ -809,7 +829,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                 double c = halo_cost(it.iy, it.iz, it.xa, it.xb);
                 const double *fc = &fcost[((size_t)it.iy * g.ntz + it.iz) * nx];
                 while (xsplit < it.xb - MIN_SPLIT) {
-                    const double cx = fc[xsplit] > 0.0 ? fc[xsplit] : COST_EMPTY_STEP;
+                    const double cx = fc[xsplit] > 0.0 ? fc[xsplit] : cost_empty;
                     if (load[cta] + c + cx > finish) break;
                     c += cx;
                     ++xsplit;
@@ -903,6 +923,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                 hdrp[1] = (uint32_t)(pc.chunk * SW_C);
                 hdrp[2] = tx1;
                 hdrp[3] = tx2;
+                out.rec_cell.push_back(full && p >= 0 && p < nx ? (int32_t)(((size_t)pc.iy * g.ntz + pc.iz) * nx + p) : -1);
                 for (int y = 0; y < TY; ++y)
                     for (int z = 0; z < TZ; ++z) cidx[y * TZ + z] = full ? g.point(p, y0 + y, z0 + z) : -1;
                 ++out.nrec;
@@ -945,7 +966,8 @@ static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables *
     if (f == m->sweep.end()) {
         rs_sweep_host h;
         rs_sweep_tables tb;
-        tb.ok = rs_sweep_build_host(m, n, ncol, g_max_planes, sweep_nctas(m), h);
+        const auto mc = m->sweep_costs.find(key);
+        tb.ok = rs_sweep_build_host(m, n, ncol, g_max_planes, sweep_nctas(m), h, mc == m->sweep_costs.end() ? nullptr : &mc->second);
         if (tb.ok) {
             tb.nitems = (int64_t)h.items.size();
             tb.nrec = h.nrec;
@@ -957,6 +979,9 @@ static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables *
             };
             RS_CUDA_TRY(up((void **)&tb.d_items, h.items.data(), h.items.size() * sizeof(int2)));
             RS_CUDA_TRY(up((void **)&tb.d_recs, h.recs.data(), h.recs.size()));
+            RS_CUDA_TRY(cudaMalloc((void **)&tb.d_step_clock, (size_t)(h.nrec + 1) * sizeof(long long)));
+            tb.host_items = h.items;
+            tb.rec_cell = h.rec_cell;
             RS_CUDA_TRY(cudaMalloc((void **)&tb.d_cycles, (h.items.size() + 2048) * sizeof(long long)));
             RS_CUDA_TRY(cudaMemset(tb.d_cycles, 0, (h.items.size() + 2048) * sizeof(long long)));
             tb.variant = sweep_variant(n);
@@ -1019,6 +1044,7 @@ rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const d
     a.items = tb->d_items, a.recs = tb->d_recs;
     a.vloc = vloc, a.psi = psi, a.hpsi = hpsi, a.ncol = (uint32_t)ncol;
     a.cycles = tb->d_cycles;
+    a.step_clock = tb->d_step_clock;
     sweep_maps maps;
     const bool tensor = ncol != SW_C || g_force_tensor;
     if (tensor) {
@@ -1073,7 +1099,7 @@ void rs_sweep_free(rs_mesh *m)
 {
     for (auto &kv : m->sweep) {
         rs_sweep_tables &t = kv.second;
-        cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles);
+        cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles), cudaFree(t.d_step_clock);
     }
     m->sweep.clear();
 }
@@ -1204,4 +1230,68 @@ int64_t rs_sweep_read_stats(const rs_mesh *cm, int n, int ncol, int64_t *out, in
         for (int k = 0; k < 4; ++k) out[5 * c + 1 + k] = t.host_stats[4 * c + k];
     }
     return nc;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Measure, don't guess: run the kernel on the caller's buffers, read the clock every CTA recorded at the end
+// of every step, and deal the work again with the measured cost of each (tile, plane) instead of the model.
+// The per-CTA residual of the model is systematic (run-to-run correlation 0.95-0.97 on B200), so it can be
+// measured once per mesh.  Synchronises `st`.
+// ---------------------------------------------------------------------------------------------
+rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const double *vloc, const double *psi, double *hpsi,
+                            int ncol, cudaStream_t st)
+{
+    rs_mesh *m = const_cast<rs_mesh *>(cm);
+    if (!rs_sweep_supported(m, n, ncol)) return RS_OK;   // the gather kernel serves this call: nothing to tune
+    const auto key = std::make_pair(n * 16 + sweep_variant(n), ncol);
+    rs_sweep_costs costs;
+    for (int round = 0; round < 2; ++round) {   // the second round measures the re-dealt work and refines it once
+        const rs_sweep_tables *tb = nullptr;
+        rs_status rc = get_tables(m, n, ncol, &tb);
+        if (rc != RS_OK) return rc;
+        if (!tb->ok) return RS_OK;
+        for (int rep = 0; rep < 3; ++rep) {
+            rc = rs_launch_sweep(m, n, w, vloc, psi, hpsi, ncol, st);
+            if (rc != RS_OK) return rc;
+        }
+        RS_CUDA_TRY(cudaStreamSynchronize(st));
+        std::vector<long long> clk((size_t)tb->nrec + 1);
+        RS_CUDA_TRY(cudaMemcpy(clk.data(), tb->d_step_clock, clk.size() * sizeof(long long), cudaMemcpyDeviceToHost));
+        size_t ncell = 0;
+        for (int32_t c : tb->rec_cell) ncell = std::max(ncell, (size_t)(c + 1));
+        const shape_rt sh = variant_shape(tb->variant);
+        const size_t cells = (size_t)((m->dims[1] + sh.TY - 1) / sh.TY) * ((m->dims[2] + SW_TZ - 1) / SW_TZ) * m->dims[0];
+        std::vector<double> sum(cells, 0.0);
+        std::vector<int> cnt(cells, 0);
+        double halo_sum = 0.0, full_sum = 0.0;
+        int64_t halo_n = 0, full_n = 0;
+        for (const int2 &it : tb->host_items)
+            for (int t = 1; t < it.y; ++t) {   // step 0 has no predecessor to difference against
+                const double d = (double)(clk[(size_t)it.x + t] - clk[(size_t)it.x + t - 1]);
+                const int32_t cell = tb->rec_cell[(size_t)it.x + t];
+                if (d <= 0.0 || d > 1e7) continue;
+                if (cell < 0) {
+                    halo_sum += d, ++halo_n;
+                } else if ((size_t)cell < cells) {
+                    sum[cell] += d, ++cnt[cell];
+                    full_sum += d, ++full_n;
+                }
+            }
+        if (!full_n || !halo_n) return RS_OK;
+        costs.full.assign(cells, 0.f);
+        for (size_t q = 0; q < cells; ++q)
+            if (cnt[q]) costs.full[q] = (float)(sum[q] / cnt[q]);
+        costs.halo = halo_sum / halo_n;
+        costs.unit = full_sum / full_n;
+        m->sweep_costs[key] = costs;
+        // drop the tables: the next use builds them with the measured costs
+        auto f = m->sweep.find(key);
+        if (f != m->sweep.end()) {
+            rs_sweep_tables &t = f->second;
+            cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles), cudaFree(t.d_step_clock);
+            m->sweep.erase(f);
+        }
+    }
+    const rs_sweep_tables *tb = nullptr;
+    return get_tables(m, n, ncol, &tb);
 }

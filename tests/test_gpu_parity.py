@@ -128,6 +128,31 @@ def test_sweep_kernel_12_warp_shape(B):
     check(g, o, problem(1).cond_denominator(psi, 4), f"12-warp shape B={B}")
 
 
+def test_autotune_keeps_parity():
+    """rs_hamiltonian_autotune re-deals the plane-sweep work from measured step costs: same results, kernel still the sweep."""
+    import torch
+
+    cfg = synthetic.config(1)
+    p = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=4)      # fresh mesh: its tables get replaced
+    B = 16
+    psi = synthetic.orbitals(cfg.seed, 0, B, p.np)
+    dev = torch.device("cuda:0")
+    states = torch.from_numpy(p.to_mesh(psi)).to(dev)
+    v = torch.from_numpy(p.v_mesh).to(dev)
+    blk = torch.empty((p.np + 1, B), dtype=torch.float64, device=dev)
+    hblk = torch.full((p.np + 1, B), 3.0, dtype=torch.float64, device=dev)
+    rs.rs_block_pack(p.mesh, states, 0, B, B, blk)
+    rs.rs_hamiltonian_autotune(p.mesh, 4, oracle.fd_coeffs(4), v, blk, hblk, B)
+    out = torch.empty_like(states)
+    rs.rs_block_unpack(p.mesh, hblk, B, B, out, 0)
+    o = problem(1).oracle_hpsi(psi, 4)
+    check(p.to_canon(out.cpu().numpy()), o, problem(1).cond_denominator(psi, 4), "autotune call itself")
+    g = p.gpu_hpsi(psi, 4, B, kernel=rs.RS_KERNEL_SWEEP)                          # re-dealt tables
+    check(g, o, problem(1).cond_denominator(psi, 4), "after autotune")
+    st = rs.rs_sweep_stats(p.mesh, 4, B)
+    assert st.shape[0] > 0 and st[:, 0].max() > 0
+
+
 def test_sweep_kernel_dirichlet_boxes():
     """Non-periodic boxes through the plane-sweep kernel: sizes that are not multiples of the 16 x 16 tile."""
     for box in [(24, 24, 24), (7, 9, 10), (1, 1, 37), (13, 1, 5), (40, 17, 33)]:
