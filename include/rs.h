@@ -155,7 +155,8 @@ const char *rs_kernel_name(const rs_mesh *mesh, int fd_order, int nst, rs_dtype 
 int64_t rs_kernel_table_bytes(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, rs_kernel kernel);
 int rs_version(void);
 /* Tuning knobs for tests and ablations (not needed for normal use); they take effect for tables built
- * afterwards.  "sweep_planes": x-slab thickness of a plane-sweep work item (default 32); "sweep_ctas":
+ * afterwards.  "sweep_planes": x-slab thickness of a plane-sweep work item (default 32), "sweep_planes_tuned": the same
+ * after rs_hamiltonian_autotune (default: the whole x extent); "sweep_ctas":
  * number of persistent CTAs (0 = one per SM); "sweep_tensor": 1 = use the 2-D tensor-map copies also for
  * 16-column blocks; "sweep_shape": 1 = run fd_order 4 on the experimental 12-warp kernel shape.
  * Unknown name -> RS_ERR_INVALID_ARG.                                                                  */

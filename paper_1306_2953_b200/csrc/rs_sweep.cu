@@ -652,10 +652,14 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
 // host: work pieces, their assignment to CTAs, and the per-step records
 // ---------------------------------------------------------------------------------------------
 static int g_max_planes = 32;   // x-slab thickness of a work item (rs_set_tuning("sweep_planes", v))
+static int g_tuned_planes = 1 << 20;   // the same once the step costs are measured (rs_set_tuning("sweep_planes_tuned", v)):
+                                       // with true costs the dealing balances whole tile columns, and fewer pieces mean
+                                       // fewer halo steps (measured on B200, config 2: 32 -> 0.148 ms, whole extent -> 0.140 ms)
 static int g_force_tensor = 0;  // rs_set_tuning("sweep_tensor", 1): use the tensor-map copies also for 16 columns (tests)
 static int g_nctas = 0;         // rs_set_tuning("sweep_ctas", v): persistent CTAs (0 = one per SM)
 static int g_shape = 0;         // rs_set_tuning("sweep_shape", 1): fd_order 4 on the 12-warp shape (experiment)
 void rs_sweep_set_max_planes(int v) { g_max_planes = v < 4 ? 4 : v; }
+void rs_sweep_set_tuned_planes(int v) { g_tuned_planes = v < 4 ? 4 : v; }
 void rs_sweep_set_force_tensor(int v) { g_force_tensor = v != 0; }
 void rs_sweep_set_nctas(int v) { g_nctas = v < 0 ? 0 : v; }
 void rs_sweep_set_shape(int v) { g_shape = v; }
@@ -967,7 +971,8 @@ static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables *
         rs_sweep_host h;
         rs_sweep_tables tb;
         const auto mc = m->sweep_costs.find(key);
-        tb.ok = rs_sweep_build_host(m, n, ncol, g_max_planes, sweep_nctas(m), h, mc == m->sweep_costs.end() ? nullptr : &mc->second);
+        const bool tuned = mc != m->sweep_costs.end();
+        tb.ok = rs_sweep_build_host(m, n, ncol, tuned ? g_tuned_planes : g_max_planes, sweep_nctas(m), h, tuned ? &mc->second : nullptr);
         if (tb.ok) {
             tb.nitems = (int64_t)h.items.size();
             tb.nrec = h.nrec;
