@@ -234,8 +234,6 @@ def main() -> None:
     blk = torch.empty((npts + 1, B), dtype=tdt, device=dev)
     hblk = torch.empty((npts + 1, B), dtype=tdt, device=dev)
     nblocks = (nst + B - 1) // B
-    kname = rs.rs_kernel_name(mesh, n, B, rsdt, kern)
-    table_bytes = rs.rs_kernel_table_bytes(mesh, n, B, rsdt, kern)
 
     apply_events = []
 
@@ -263,6 +261,8 @@ def main() -> None:
         rs.rs_block_pack(mesh, states, 0, min(B, nst), B, blk)
         rs.rs_hamiltonian_autotune(mesh, n, coeffs, v, blk, hblk, B)
     t_tune = time.perf_counter() - t
+    kname = rs.rs_kernel_name(mesh, n, B, rsdt, kern)
+    table_bytes = rs.rs_kernel_table_bytes(mesh, n, B, rsdt, kern)     # of the tables in use (after the re-deal)
     for _ in range(args.warmup):
         step(False)
     barrier()
