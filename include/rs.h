@@ -158,7 +158,9 @@ int rs_version(void);
  * afterwards.  "sweep_planes": x-slab thickness of a plane-sweep work item (default 32), "sweep_planes_tuned": the same
  * after rs_hamiltonian_autotune (default: the whole x extent); "sweep_ctas":
  * number of persistent CTAs (0 = one per SM); "sweep_tensor": 1 = use the 2-D tensor-map copies also for
- * 16-column blocks; "sweep_shape": 1 = run fd_order 4 on the experimental 12-warp kernel shape.
+ * 16-column blocks; "sweep_shape": 1 = run fd_order 4 on the experimental 12-warp kernel shape; "sweep_min_split": fewest
+ * output planes of a work piece cut off when dealing (default 3); "sweep_tune_rounds": measure / re-deal rounds of
+ * rs_hamiltonian_autotune (default 3).
  * Unknown name -> RS_ERR_INVALID_ARG.                                                                  */
 rs_status rs_set_tuning(const char *name, int value);
 /* Host-only diagnostic (no device needed): build the plane-sweep kernel's compact records for (mesh,

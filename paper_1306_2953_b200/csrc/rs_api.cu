@@ -191,6 +191,8 @@ void rs_sweep_set_force_tensor(int v);
 void rs_sweep_set_nctas(int v);
 void rs_sweep_set_shape(int v);
 void rs_sweep_set_tuned_planes(int v);
+void rs_sweep_set_min_split(int v);
+void rs_sweep_set_tune_rounds(int v);
 std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, int64_t *stats);
 
 extern "C" rs_status rs_set_tuning(const char *name, int value)
@@ -205,6 +207,14 @@ extern "C" rs_status rs_set_tuning(const char *name, int value)
     }
     if (name && std::strcmp(name, "sweep_planes_tuned") == 0) {
         rs_sweep_set_tuned_planes(value);
+        return RS_OK;
+    }
+    if (name && std::strcmp(name, "sweep_min_split") == 0) {
+        rs_sweep_set_min_split(value);
+        return RS_OK;
+    }
+    if (name && std::strcmp(name, "sweep_tune_rounds") == 0) {
+        rs_sweep_set_tune_rounds(value);
         return RS_OK;
     }
     if (name && std::strcmp(name, "sweep_shape") == 0) {

@@ -657,12 +657,16 @@ static int g_tuned_planes = 1 << 20;   // the same once the step costs are measu
                                        // fewer halo steps (measured on B200, config 2: 32 -> 0.148 ms, whole extent -> 0.140 ms)
 static int g_force_tensor = 0;  // rs_set_tuning("sweep_tensor", 1): use the tensor-map copies also for 16 columns (tests)
 static int g_nctas = 0;         // rs_set_tuning("sweep_ctas", v): persistent CTAs (0 = one per SM)
+static int g_min_split = 3;     // rs_set_tuning("sweep_min_split", v): fewest output planes of a piece cut off by the dealing
+static int g_tune_rounds = 3;   // rs_set_tuning("sweep_tune_rounds", v): measure / re-deal rounds of rs_hamiltonian_autotune
 static int g_shape = 0;         // rs_set_tuning("sweep_shape", 1): fd_order 4 on the 12-warp shape (experiment)
 void rs_sweep_set_max_planes(int v) { g_max_planes = v < 4 ? 4 : v; }
 void rs_sweep_set_tuned_planes(int v) { g_tuned_planes = v < 4 ? 4 : v; }
 void rs_sweep_set_force_tensor(int v) { g_force_tensor = v != 0; }
 void rs_sweep_set_nctas(int v) { g_nctas = v < 0 ? 0 : v; }
 void rs_sweep_set_shape(int v) { g_shape = v; }
+void rs_sweep_set_min_split(int v) { g_min_split = v < 1 ? 1 : v; }
+void rs_sweep_set_tune_rounds(int v) { g_tune_rounds = v < 1 ? 1 : v; }
 
 namespace {
 enum { VARIANT_N4 = 0, VARIANT_N6 = 1, VARIANT_N4W12 = 2, VARIANT_NONE = -1 };
@@ -805,7 +809,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
         pieces.assign(nctas, {});
         load.assign(nctas, 0.0);
         std::vector<char> closed(nctas, 0);   // CTAs that cannot take another piece without overshooting
-        const int MIN_SPLIT = 6;              // output planes: below this the 2 N halo steps dominate
+                const int MIN_SPLIT = g_min_split;    // output planes: below this the 2 N halo steps dominate
         auto least_loaded = [&](bool open_only) {
             int best = -1;
             for (int c = 0; c < nctas; ++c)
@@ -1250,7 +1254,7 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
     if (!rs_sweep_supported(m, n, ncol)) return RS_OK;   // the gather kernel serves this call: nothing to tune
     const auto key = std::make_pair(n * 16 + sweep_variant(n), ncol);
     rs_sweep_costs costs;
-    for (int round = 0; round < 2; ++round) {   // the second round measures the re-dealt work and refines it once
+    for (int round = 0; round < g_tune_rounds; ++round) {   // later rounds measure the re-dealt work and refine it
         const rs_sweep_tables *tb = nullptr;
         rs_status rc = get_tables(m, n, ncol, &tb);
         if (rc != RS_OK) return rc;
