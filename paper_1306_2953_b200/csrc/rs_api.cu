@@ -82,7 +82,7 @@ extern "C" rs_status rs_hamiltonian_autotune(const rs_mesh *m, int n, const doub
     std::memset(&w, 0, sizeof(w));
     for (int k = 0; k <= n; ++k) w.w[k] = -0.5 * coeffs[k] / (m->h * m->h);
     const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
-    if (resolve_kernel(m, n, ncol, RS_KERNEL_AUTO) != RS_KERNEL_SWEEP)   // gather kernel: nothing to tune, just apply
+    if (!rs_sweep_usable(m, n, ncol))   // only the gather kernel can serve this call: nothing to tune, just apply
         return rs_hamiltonian_apply(m, n, coeffs, vloc, psi, hpsi, nst, dtype, stream);
     return rs_sweep_autotune(m, n, w, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
 }

@@ -153,6 +153,31 @@ def test_autotune_keeps_parity():
     assert st.shape[0] > 0 and st[:, 0].max() > 0
 
 
+@pytest.mark.parametrize("seed,n,B", [(0, 4, 16), (1, 4, 32), (2, 6, 16), (3, 6, 32)])
+def test_sweep_kernel_ragged_clusters(seed, n, B):
+    """Small spheres scattered so that z-rows break into several copy runs of odd lengths and most tiles are nearly
+    empty: 1-D bulk copies (B = 16) and overlapping 2-D tensor boxes (B = 32), before and after the autotuned re-deal."""
+    rng = np.random.default_rng(seed)
+    nc = int(rng.integers(4, 12))
+    centers = rng.uniform(0.0, 9.0, (nc, 3))
+    charges = rng.choice(np.array([1.0, 4.0, 6.0]), nc)
+    p = Problem(centers, charges, float(rng.uniform(1.3, 2.6)), 0.3, max_n=6)
+    psi = rng.standard_normal((B + 5, p.np))
+    o = p.oracle_hpsi(psi, n)
+    den = p.cond_denominator(psi, n)
+    check(_run(p, psi, n, B, "sweep"), o, den, f"ragged seed {seed} n={n} B={B}")
+    import torch
+    blk = torch.zeros((p.np + 1, B), dtype=torch.float64, device="cuda")
+    hblk = torch.empty_like(blk)
+    v = torch.from_numpy(p.v_mesh).cuda()
+    rs.rs_set_tuning("sweep_planes_tuned", 7)            # short pieces after the re-deal as well
+    try:
+        rs.rs_hamiltonian_autotune(p.mesh, n, oracle.fd_coeffs(n), v, blk, hblk, B)
+    finally:
+        rs.rs_set_tuning("sweep_planes_tuned", 1 << 20)
+    check(_run(p, psi, n, B, "sweep"), o, den, f"ragged seed {seed} n={n} B={B} after autotune")
+
+
 def test_sweep_kernel_dirichlet_boxes():
     """Non-periodic boxes through the plane-sweep kernel: sizes that are not multiples of the 16 x 16 tile."""
     for box in [(24, 24, 24), (7, 9, 10), (1, 1, 37), (13, 1, 5), (40, 17, 33)]:

@@ -233,3 +233,18 @@ def test_sweep_selfcheck_on_boxes_and_unsupported_calls():
     with pytest.raises(rs.RsError) as e:
         rs.rs_sweep_selfcheck(mesh, 5, 16)                                          # fd_order 5: gather kernel only
     assert e.value.status == rs.RS_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_sweep_records_on_random_sparse_clusters(seed):
+    """Ragged meshes: small spheres scattered so that z-rows break into several runs, tiles are mostly empty and
+    pieces are short; the record replay must still expand to the plain table (both kernel shapes, odd CTA counts)."""
+    rng = np.random.default_rng(seed)
+    nc = int(rng.integers(3, 12))
+    centers = rng.uniform(0.0, 9.0, (nc, 3))
+    radius = float(rng.uniform(1.1, 2.6))
+    mesh = rs.rs_mesh_create(centers, radius, 0.3, 6)
+    for n in (4, 6):
+        for nst, planes, nctas in ((16, int(rng.integers(4, 40)), int(rng.integers(1, 200))), (32, 1 << 20, 148)):
+            st = rs.rs_sweep_selfcheck(mesh, n, nst, rs.RS_REAL64, planes, nctas)
+            assert st["records"] > 0
