@@ -181,10 +181,10 @@ def rs_sweep_stats(mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, max_ct
 
 def rs_sweep_selfcheck(mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, max_planes: int = 32, nctas: int = 148) -> dict:
     """Host-only replay of the plane-sweep records against the plain neighbour table; raises on a discrepancy."""
-    st = (C.c_int64 * 6)()
+    st = (C.c_int64 * 8)()
     _check(_lib.rs_sweep_selfcheck(mesh.handle, fd_order, nst, dtype, max_planes, nctas, st))
     return {"nctas": st[0], "records": st[1], "pieces": st[2], "cost_max": st[3] / 1000.0, "cost_mean": st[4] / 1000.0,
-            "table_bytes": st[5]}
+            "table_bytes": st[5], "fill_slots": st[6], "copy_runs": st[7]}
 
 
 def rs_mesh_create(centers, radius: float, spacing: float, max_fd_order: int = 4,

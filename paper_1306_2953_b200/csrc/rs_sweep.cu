@@ -236,7 +236,8 @@ struct sweep_maps {
 
 // Optional timeline of one CTA (development builds only, -DSW_TRACE): clock64 stamps per step after the per-CTA ticks.
 #ifndef SW_EXP
-#define SW_EXP 0   // development builds: bit 0 drops the FULL-mode stores, bit 1 the tensor-memory traffic, bit 2 the z/y loads
+#define SW_EXP 0   // development builds: bit 0 drops the FULL-mode stores, bit 1 the tensor-memory traffic, bit 2 the z/y loads,
+                   // bit 3 stamps the producer instead of the consumer, bit 6 makes the consumers only wait and release
 #endif
 #ifdef SW_TRACE
 #define SW_STAMP(cond, t, k) do { if ((cond) && blockIdx.x == SW_TRACE && (t) < 256) a.cycles[gridDim.x + (t) * 8 + (k)] = clock64(); } while (0)
@@ -455,7 +456,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 5);
             const unsigned char *sp = smem + (size_t)stage * S::STAGE_BYTES;
             const uint2 hdr = *reinterpret_cast<const uint2 *>(sp + S::HDR_OFF);   // {modes | flags, column offset}
-            const int mode = (int)((hdr.x >> (2 * warp)) & 3u);
+            const int mode = (SW_EXP & 64) ? MODE_EMPTY : (int)((hdr.x >> (2 * warp)) & 3u);   // development, bit 6: consumers only wait and release
             const double *pb = reinterpret_cast<const double *>(sp + b0);
 
             // store offsets of the outputs this step completes (plane t - N), staged by the producer; -1: none
@@ -1215,6 +1216,13 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
         stats[0] = nctas, stats[1] = h.nrec, stats[2] = npieces;
         stats[3] = (int64_t)(h.cost_max * 1000), stats[4] = (int64_t)(h.cost_mean * 1000);
         stats[5] = (int64_t)(h.items.size() * sizeof(int2) + h.recs.size());
+        int64_t nfill = 0, nruns = 0;
+        for (int64_t r = 0; r < h.nrec; ++r) {
+            const unsigned char *rec = h.recs.data() + (size_t)r * sh.rec_bytes;
+            for (int q = 0; q < 18; ++q) nfill += __builtin_popcount(reinterpret_cast<const uint32_t *>(rec + SW_REC_FILL)[q]);
+            for (int q = 0; q < SW_MAXRUN; ++q) nruns += (reinterpret_cast<const uint2 *>(rec + SW_REC_RUNS)[q].y >> 16) != 0;
+        }
+        stats[6] = nfill, stats[7] = nruns;
     }
     return std::string();
 }
