@@ -134,7 +134,9 @@ rs_status rs_hamiltonian_apply_v(const rs_mesh *mesh, int fd_order, const double
  * caller's buffers (arguments as rs_hamiltonian_apply; hpsi receives H psi), reads back the clock each persistent
  * CTA recorded at the end of every plane, and deals the work to the CTAs again using the measured cost of every
  * (tile, plane) instead of the built-in cost model.  Later rs_hamiltonian_apply calls use the re-dealt tables; results
- * are unchanged up to rounding order.  SYNCHRONISES `stream`.  A call that the gather kernel serves is just applied. */
+ * are unchanged up to rounding order.  SYNCHRONISES `stream` and replaces the mesh's device tables: no other call
+ * on this mesh may be in flight on another stream or thread.  A call that only the gather kernel can serve is just
+ * applied.  (The library keeps no global state besides the tuning knobs; a mesh handle is not thread-safe.)       */
 rs_status rs_hamiltonian_autotune(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
                                   const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
                                   rs_dtype dtype, void *stream);
