@@ -170,7 +170,8 @@ rs_status rs_set_tuning(const char *name, int value);
  * symbolically and verify that they expand to exactly the plain table of rs_mesh_get_index_map and that
  * every (point, 16-column slice) is produced exactly once (reading S15 of DESIGN.md).  stats_host (may be
  * NULL) receives 8 values: {nctas, records, work pieces, modelled cost of the busiest CTA x1000, of the average
- * CTA x1000, table bytes, slots zero-filled over all records, copy runs over all records}.  RS_ERR_UNSUPPORTED if the sweep kernel cannot serve the call; a discrepancy ->
+ * CTA x1000, table bytes, slots zero-filled over all records, copy runs over all records}.  RS_ERR_UNSUPPORTED if
+ * the sweep kernel cannot serve the call; a discrepancy ->
  * RS_ERR_INVALID_ARG with the first offending (CTA, step, point, arm) in rs_last_error().               */
 rs_status rs_sweep_selfcheck(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, int max_planes, int nctas,
                              int64_t *stats_host);
