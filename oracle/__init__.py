@@ -15,15 +15,16 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.c")
+_SRC_NEXT = os.path.join(_HERE, "oracle_next.c")      # SURVEY.md section 8(f) rows (block BLAS-1, overlap, non-local)
 _SO = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> str:
     """Compile oracle.c with gcc (-O2, no FMA contraction so the summation order is the source's)."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_NEXT)):
         cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c99",
-               "-o", _SO, _SRC, "-lm"]
+               "-o", _SO, _SRC, _SRC_NEXT, "-lm"]
         subprocess.run(cmd, check=True)
     return _SO
 
@@ -53,6 +54,19 @@ def lib():
         L.orc_block_pack.restype = None
         L.orc_block_unpack.argtypes = [dp, C.c_int, C.c_int, C.c_int64, dp, C.c_int64, C.c_int, C.c_int]
         L.orc_block_unpack.restype = None
+        i32p = C.POINTER(C.c_int32)
+        L.orc_block_dot.argtypes = [dp, dp, C.c_int64, C.c_int, C.c_int, dp]
+        L.orc_block_dot.restype = None
+        L.orc_block_axpy.argtypes = [dp, dp, dp, C.c_int64, C.c_int, C.c_int]
+        L.orc_block_axpy.restype = None
+        L.orc_block_residual.argtypes = [dp, dp, dp, C.c_int64, C.c_int, C.c_int, dp]
+        L.orc_block_residual.restype = None
+        L.orc_overlap.argtypes = [dp, C.c_int, dp, C.c_int, C.c_int64, C.c_int, dp]
+        L.orc_overlap.restype = None
+        L.orc_sphere_points.argtypes = [i32p, C.c_int64, C.c_double, dp, C.c_double, i64p]
+        L.orc_sphere_points.restype = C.c_int64
+        L.orc_nonlocal.argtypes = [C.c_int, i64p, i64p, i64p, dp, C.c_int, C.c_double, dp, dp, C.c_int64, C.c_int, C.c_int]
+        L.orc_nonlocal.restype = None
         _lib = L
     return _lib
 
@@ -211,3 +225,104 @@ def block_unpack(block: np.ndarray, nst_in_block: int, npts: int, states: np.nda
     assert states.flags.c_contiguous and block.flags.c_contiguous and states.dtype == block.dtype
     lib().orc_block_unpack(block.ctypes.data_as(C.POINTER(C.c_double)), block.shape[1], nst_in_block, npts,
                            states.ctypes.data_as(C.POINTER(C.c_double)), states.shape[1], ist0, lanes)
+
+
+# ---- oracle_next.c ---------------------------------------------------------------
+def _as2d(a):
+    a = np.ascontiguousarray(a)
+    return a[None, :] if a.ndim == 1 else a
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def block_dot(a: np.ndarray, b: np.ndarray) -> np.ndarray:
+    """out[j] = sum_p conj(a[j][p]) b[j][p]   (sec. VIII; plain sums, reading S11)."""
+    a, b = _as2d(a), _as2d(b)
+    assert a.shape == b.shape and a.dtype == b.dtype
+    lanes = 2 if np.iscomplexobj(a) else 1
+    out = np.zeros(a.shape[0], dtype=a.dtype)
+    lib().orc_block_dot(_dp(a), _dp(b), a.shape[1], a.shape[0], lanes, _dp(out))
+    return out
+
+
+def block_axpy(alpha: np.ndarray, x: np.ndarray, y: np.ndarray) -> np.ndarray:
+    """returns y + alpha_j x_j per orbital (linear combination)."""
+    x = _as2d(x)
+    y = np.array(_as2d(y), copy=True, order="C")
+    assert x.shape == y.shape and x.dtype == y.dtype
+    lanes = 2 if np.iscomplexobj(x) else 1
+    alpha = np.ascontiguousarray(alpha, dtype=x.dtype)
+    assert alpha.shape == (x.shape[0],)
+    lib().orc_block_axpy(_dp(alpha), _dp(x), _dp(y), x.shape[1], x.shape[0], lanes)
+    return y
+
+
+def block_residual(hpsi_: np.ndarray, psi: np.ndarray, eps: np.ndarray) -> np.ndarray:
+    """r_j = (H psi)_j - eps_j psi_j, eps real (RMM-DIIS residual)."""
+    hpsi_, psi = _as2d(hpsi_), _as2d(psi)
+    assert hpsi_.shape == psi.shape and hpsi_.dtype == psi.dtype
+    lanes = 2 if np.iscomplexobj(psi) else 1
+    eps = np.ascontiguousarray(eps, dtype=np.float64)
+    assert eps.shape == (psi.shape[0],)
+    r = np.empty_like(psi)
+    lib().orc_block_residual(_dp(hpsi_), _dp(psi), _dp(eps), psi.shape[1], psi.shape[0], lanes, _dp(r))
+    return r
+
+
+def overlap(a: np.ndarray, b: np.ndarray) -> np.ndarray:
+    """M[j][k] = sum_p conj(a[j][p]) b[k][p]: S (eq. 5, b = a) or h (eq. 7, b = H a)."""
+    a, b = _as2d(a), _as2d(b)
+    assert a.shape[1] == b.shape[1] and a.dtype == b.dtype
+    lanes = 2 if np.iscomplexobj(a) else 1
+    M = np.zeros((a.shape[0], b.shape[0]), dtype=a.dtype)
+    lib().orc_overlap(_dp(a), a.shape[0], _dp(b), b.shape[0], a.shape[1], lanes, _dp(M))
+    return M
+
+
+@dataclass
+class Projectors:
+    """Non-local projector data in the oracle's canonical point order (eq. 4)."""
+    off: np.ndarray      # [natoms] int64 offsets into idx / gamma
+    npts: np.ndarray     # [natoms] int64 sphere sizes
+    idx: np.ndarray      # [sum npts] int64 canonical point indices, ascending per atom
+    gamma: np.ndarray    # [sum npts][nlm] float64 projector values (INPUT)
+    nlm: int
+
+
+def sphere_points(mesh: Mesh, center, rc: float) -> np.ndarray:
+    """canonical indices of the mesh points in the closed ball of radius rc around `center` (ascending)."""
+    ijk = np.ascontiguousarray(mesh.ijk(), dtype=np.int32)
+    ctr = np.ascontiguousarray(center, dtype=np.float64)
+    n = lib().orc_sphere_points(ijk.ctypes.data_as(C.POINTER(C.c_int32)), mesh.npoints, mesh.spacing, _dp(ctr), rc, None)
+    idx = np.empty(n, dtype=np.int64)
+    lib().orc_sphere_points(ijk.ctypes.data_as(C.POINTER(C.c_int32)), mesh.npoints, mesh.spacing, _dp(ctr), rc,
+                            idx.ctypes.data_as(C.POINTER(C.c_int64)))
+    return idx
+
+
+def make_projectors(mesh: Mesh, centers: np.ndarray, rc: float, values_at) -> Projectors:
+    """values_at(xyz_relative [n][3]) -> [n][nlm]: the projector values are an input supplied by the caller."""
+    centers = np.ascontiguousarray(centers, dtype=np.float64).reshape(-1, 3)
+    xyz = mesh.xyz()
+    idxs, gam = [], []
+    for A in range(centers.shape[0]):
+        ix = sphere_points(mesh, centers[A], rc)
+        idxs.append(ix)
+        gam.append(np.ascontiguousarray(values_at(xyz[ix] - centers[A]), dtype=np.float64).reshape(ix.size, -1))
+    npts = np.array([i.size for i in idxs], dtype=np.int64)
+    off = np.concatenate([[0], np.cumsum(npts)[:-1]]).astype(np.int64)
+    nlm = gam[0].shape[1]
+    return Projectors(off, npts, np.concatenate(idxs).astype(np.int64), np.ascontiguousarray(np.concatenate(gam, axis=0)), nlm)
+
+
+def nonlocal_apply(mesh: Mesh, proj: Projectors, psi: np.ndarray, out: np.ndarray | None = None) -> np.ndarray:
+    """out + V_nl psi (eq. 4; integral = h^3 * lattice sum); out defaults to zeros."""
+    psi = _as2d(psi)
+    lanes = 2 if np.iscomplexobj(psi) else 1
+    res = np.zeros_like(psi) if out is None else np.array(_as2d(out), copy=True, order="C")
+    lib().orc_nonlocal(int(proj.off.size), proj.off.ctypes.data_as(C.POINTER(C.c_int64)),
+                       proj.npts.ctypes.data_as(C.POINTER(C.c_int64)), proj.idx.ctypes.data_as(C.POINTER(C.c_int64)),
+                       _dp(proj.gamma), proj.nlm, mesh.spacing ** 3, _dp(psi), _dp(res), psi.shape[1], psi.shape[0], lanes)
+    return res

@@ -113,6 +113,25 @@ def vloc_at(xyz: np.ndarray, centers: np.ndarray, charges: np.ndarray, chunk: in
     return out
 
 
+def projector_values(xyz_rel: np.ndarray, lmax: int = 1, sigma: float = 0.7) -> np.ndarray:
+    """Synthetic stand-ins for the pseudopotential projectors gamma_lm(r - R_A) of PAPER.md:181 (eq. 4), whose real
+    data are not available: a Gaussian exp(-r^2/(2 sigma^2)) times the real solid harmonics up to lmax <= 2
+    (1; x, y, z; xy, yz, zx, x^2-y^2, 3z^2-r^2).  An INPUT of the path, sampled at caller-supplied coordinates
+    relative to the atom; the caller decides which points lie inside the cut-off sphere.  Returns [n][(lmax+1)^2]."""
+    p = np.ascontiguousarray(xyz_rel, dtype=np.float64).reshape(-1, 3)
+    x, y, z = p[:, 0], p[:, 1], p[:, 2]
+    r2 = x * x + y * y + z * z
+    g = np.exp(-r2 / (2.0 * sigma * sigma))
+    cols = [np.ones_like(x)]
+    if lmax >= 1:
+        cols += [x, y, z]
+    if lmax >= 2:
+        cols += [x * y, y * z, z * x, x * x - y * y, 3.0 * z * z - r2]
+    if lmax > 2:
+        raise ValueError("lmax <= 2")
+    return np.stack(cols, axis=1) * g[:, None]
+
+
 def orbital(seed: int, ist: int, npts: int, is_complex: bool = False) -> np.ndarray:
     """Orbital `ist` as i.i.d. N(0,1) values in canonical (lexicographic i,j,k) point order;
     complex: a second draw of npts for the imaginary part."""
