@@ -1,14 +1,16 @@
 #!/usr/bin/env python
 """bench.py -- H psi throughput on the synthetic molecule-shaped meshes (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--block 16] [--sweep]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--block 16] [--no-sweep]
     python bench.py --impl reference ...          # the CPU oracle on the host cores, same metric
 
 A "step" is one pass of the whole hot path over one batch: for every block of B orbitals,
 rs_block_pack -> rs_hamiltonian_apply -> rs_block_unpack (steps a4-a7 of DESIGN.md); the mesh tables
 (a1-a3) are built once per geometry before the timed region and their wall time is reported.
 `value` = nst * np * (2*(6n+1)+2) flops / step time with all inputs resident in HBM; `e2e` is the same
-metric through rs_hamiltonian_apply_states_host with pinned HOST buffers (H2D + D2H inside).
+metric through rs_hamiltonian_apply_states_stream with pinned HOST buffers (H2D + D2H inside); its output
+is compared with the oracle on sampled orbitals.  The line also carries the apply-alone block-size sweep
+(the metric's axis), the tuned and un-tuned kernel times, and the oracle on 1 core and on all cores.
 Prints ONE JSON line on rank 0.  See DESIGN.md "Measurement" for the byte accounting.
 """
 from __future__ import annotations
@@ -121,7 +123,7 @@ def cpu_oracle_leg(cfg, n: int, seconds_budget: float = 20.0, steps: int = 1, wa
     probe = synthetic.orbitals(cfg.seed, 0, 1, om.npoints, cfg.is_complex)
     t = time.perf_counter()
     oracle.hpsi(om, n, c, v, probe, nthreads=1)
-    t_one = time.perf_counter() - t
+    t_one = time.perf_counter() - t          # one orbital on ONE core: the 1-core baseline (cost is linear in orbitals)
     nsample = int(max(cores, min(cfg.nst, cores * max(1.0, seconds_budget / max(t_one, 1e-3)) // max(1, steps + warmup))))
     nsample = max(cores, (nsample // cores) * cores)
     nsample = min(nsample, max(cores, cfg.nst))
@@ -138,6 +140,8 @@ def cpu_oracle_leg(cfg, n: int, seconds_budget: float = 20.0, steps: int = 1, wa
     return {"value": gf, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{nsample} of {cfg.nst} orbitals of config {cfg.index} (np={om.npoints}, fd_order={n}), "
                       f"{cores} OpenMP threads over orbitals, {dt:.2f} s/step",
+            "one_core": {"value": om.npoints * flops_per_output(n) * lanes / t_one / 1e9, "unit": UNIT, "cores": 1,
+                         "sample": f"1 orbital of config {cfg.index}, single thread, {t_one:.2f} s"},
             "ms_per_step": dt * 1e3, "npoints": om.npoints, "nsample": nsample}
 
 
@@ -152,20 +156,46 @@ def run_reference(args) -> None:
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": leg["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "c128" if cfg.is_complex else "f64", "data": "synthetic",
             "config": workload_config(cfg, n, args.block, leg["npoints"]),
-            "cpu_baseline": {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "cpu_baseline": {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample", "one_core")},
             "e2e": {"value": leg["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
 
-def workload_config(cfg, n, B, npts) -> dict:
+def workload_config(cfg, n, B, npts, nst=None) -> dict:
+    nst = cfg.nst if nst is None else nst
+    note = "" if nst == cfg.nst else f" (REDUCED from the config's {cfg.nst} by --nst: not the named workload)"
     return {"workload": f"configs[{cfg.index}] {cfg.name}: {cfg.centers.shape[0]} centres, R={cfg.radius}, "
-                        f"h={cfg.spacing}, np={npts}, nst={cfg.nst} {'complex' if cfg.is_complex else 'real'} fp64",
-            "fd_order": n, "block_size": B, "npoints": int(npts), "nst": cfg.nst,
+                        f"h={cfg.spacing}, np={npts}, nst={nst} {'complex' if cfg.is_complex else 'real'} fp64{note}",
+            "fd_order": n, "block_size": B, "npoints": int(npts), "nst": nst,
             "l2": "inputs larger than L2 (per-orbital states + blocks >> 126 MB); no explicit flush"}
 
 
 # ------------------------------------------------------------------------------------------------
+def time_apply(rs, torch, mesh, n, coeffs, v, b1, b2, Bs, kern, reps):
+    """Mean duration (ms) of `reps` back-to-back apply launches, CUDA events on torch's current stream."""
+    for _ in range(3):
+        rs.rs_hamiltonian_apply(mesh, n, coeffs, v, b1, b2, Bs, kernel=kern)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(reps):
+        rs.rs_hamiltonian_apply(mesh, n, coeffs, v, b1, b2, Bs, kernel=kern)
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def traffic_rows() -> dict:
+    """DRAM bytes per launch from the committed `ncu --set full` captures (profiles/traffic.csv): NOT measured by this
+    run (a number taken under a profiler is never a bench value); each row names its capture and commit."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return {}
+    return {row["key"]: row for row in csv.DictReader(open(path))}
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -175,9 +205,10 @@ def main() -> None:
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--block", type=int, default=16)
     ap.add_argument("--fd-order", type=int, default=0)
-    ap.add_argument("--nst", type=int, default=0, help="override the orbital count (debugging only; invalidates the number)")
+    ap.add_argument("--nst", type=int, default=0, help="override the orbital count (debugging only; the line says so)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "sweep"])
-    ap.add_argument("--sweep", action="store_true", help="also time apply alone for every block size of the config")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the apply-alone block-size sweep (the metric's axis)")
+    ap.add_argument("--sweep", action="store_true", help="(default now; kept for old command lines)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-autotune", action="store_true", help="skip rs_hamiltonian_autotune (work dealt by the built-in cost model)")
@@ -211,6 +242,8 @@ def main() -> None:
     rsdt = rs.RS_COMPLEX128 if is_c else rs.RS_REAL64
     tdt = torch.complex128 if is_c else torch.float64
     lanes = 2 if is_c else 1
+    conv = 4 if is_c else 1          # the metric's flop convention for complex (BASELINE.json); executed arithmetic is 2x real (S12)
+    tune = not args.no_autotune and args.kernel != "gather"
 
     # ---- once per geometry: mesh tables (a1-a3), potential, inputs --------------------------------
     t = time.perf_counter()
@@ -255,10 +288,15 @@ def main() -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # once per geometry, like the mesh tables: let the library measure its own per-plane costs and re-deal the work
+    # once per geometry, like the mesh tables: build the neighbour structure, then let the library measure its own
+    # per-plane costs and re-deal the work (rs_hamiltonian_autotune); the un-tuned time is reported beside the tuned one
     t = time.perf_counter()
-    if not args.no_autotune and args.kernel != "gather":
-        rs.rs_block_pack(mesh, states, 0, min(B, nst), B, blk)
+    rs.rs_hamiltonian_prepare(mesh, n, B, rsdt)
+    t_prepare = time.perf_counter() - t
+    rs.rs_block_pack(mesh, states, 0, min(B, nst), B, blk)
+    untuned_ms = time_apply(rs, torch, mesh, n, coeffs, v, blk, hblk, B, kern, 20)
+    t = time.perf_counter()
+    if tune:
         rs.rs_hamiltonian_autotune(mesh, n, coeffs, v, blk, hblk, B)
     t_tune = time.perf_counter() - t
     kname = rs.rs_kernel_name(mesh, n, B, rsdt, kern)
@@ -286,7 +324,7 @@ def main() -> None:
         ms_total = float(tt.item())
     clocks = sampler.stop(t0w, t1w) if rank == 0 else None
     ms_step = ms_total / args.steps
-    fl_step = nst * npts * flops_per_output(n) * (4 if is_c else 1)     # metric convention: 4x for complex
+    fl_step = nst * npts * flops_per_output(n) * conv                   # metric convention: 4x for complex
     value = world * fl_step / (ms_step * 1e-3) / 1e9
 
     apply_ms = float(np.mean([a.elapsed_time(b) for a, b in apply_events]))
@@ -296,56 +334,75 @@ def main() -> None:
     roofline = {"bound": "hbm", "kernel": f"rs_hamiltonian_apply[{kname}] B={B} n={n}", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_8TBs": achieved / 8000.0,
                 "peak_source": peak_src, "traffic": None, "algorithmic_bytes_per_launch": alg_bytes,
-                "apply_ms_per_launch": apply_ms, "apply_share_of_step": apply_ms * nblocks / ms_step,
-                "apply_gflops": B * npts * flops_per_output(n) * (4 if is_c else 1) / (apply_ms * 1e-3) / 1e9}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(traffic_file):      # dram bytes per launch from the committed ncu --set full capture
-        import csv
-        key = f"config{cfg.index}_B{B}_n{n}_{kname}"
-        for row in csv.DictReader(open(traffic_file)):
-            if row["key"] == key:
-                roofline["traffic"] = int(row["dram_bytes_per_launch"])
+                "apply_ms_per_launch": apply_ms, "apply_ms_per_launch_untuned": untuned_ms,
+                "apply_share_of_step": apply_ms * nblocks / ms_step,
+                "apply_gflops": B * npts * flops_per_output(n) * conv / (apply_ms * 1e-3) / 1e9,
+                "apply_gflops_executed": B * npts * flops_per_output(n) * lanes / (apply_ms * 1e-3) / 1e9}
+    traffic = traffic_rows()
+    row = traffic.get(f"config{cfg.index}_B{B}_n{n}_{kname}")
+    if row:    # from a committed ncu capture of this kernel, not from this run
+        roofline.update({"traffic": int(row["dram_read_bytes"]) + int(row["dram_write_bytes"]),
+                         "traffic_read": int(row["dram_read_bytes"]), "traffic_write": int(row["dram_write_bytes"]),
+                         "traffic_compulsory_read": npts * (8 * B * lanes + 8) + table_bytes,
+                         "traffic_compulsory_write": npts * 8 * B * lanes,
+                         "traffic_source": f"{row['capture']} (ncu --set full, commit {row['commit']}); not measured by this run"})
+
+    # ---- the caller that keeps psi in the block layout (the paper's storage format): apply alone over all blocks
+    blocked = None
+    if rank == 0:
+        for _ in range(2):
+            for _k in range(nblocks):
+                rs.rs_hamiltonian_apply(mesh, n, coeffs, v, blk, hblk, B, kernel=kern)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(args.steps):
+            for _k in range(nblocks):
+                rs.rs_hamiltonian_apply(mesh, n, coeffs, v, blk, hblk, B, kernel=kern)
+        b.record()
+        torch.cuda.synchronize()
+        msb = a.elapsed_time(b) / args.steps
+        blocked = {"value": fl_step / (msb * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": msb,
+                   "note": "apply over all blocks, psi kept blocked (no pack / unpack); one block buffer pair reused: "
+                           f"{2 * blk.numel() * blk.element_size() / 1e6:.0f} MB per launch vs 126 MB L2"}
 
     # ---- block-size sweep of the apply kernel alone (the metric is "vs orbital block size") -------
     sweep = None
-    if args.sweep and rank == 0:
+    if not args.no_sweep and rank == 0:
         sweep = []
         for Bs in cfg.block_sizes:
             b1 = torch.empty((npts + 1, Bs), dtype=tdt, device=dev)
             b2 = torch.empty((npts + 1, Bs), dtype=tdt, device=dev)
             rs.rs_block_pack(mesh, states, 0, min(Bs, nst), Bs, b1)
             reps = max(3, min(50, int(nst // Bs)))
-            if not args.no_autotune and args.kernel != "gather":
+            rs.rs_hamiltonian_prepare(mesh, n, Bs, rsdt)
+            ms_untuned = time_apply(rs, torch, mesh, n, coeffs, v, b1, b2, Bs, kern, reps) if Bs != B else untuned_ms
+            if tune and Bs != B:
                 rs.rs_hamiltonian_autotune(mesh, n, coeffs, v, b1, b2, Bs)
-            for _ in range(3):
-                rs.rs_hamiltonian_apply(mesh, n, coeffs, v, b1, b2, Bs, kernel=kern)
-            torch.cuda.synchronize()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            for _ in range(reps):
-                rs.rs_hamiltonian_apply(mesh, n, coeffs, v, b1, b2, Bs, kernel=kern)
-            b.record()
-            torch.cuda.synchronize()
-            ms = a.elapsed_time(b) / reps
+            ms = time_apply(rs, torch, mesh, n, coeffs, v, b1, b2, Bs, kern, reps)
+            kn = rs.rs_kernel_name(mesh, n, Bs, rsdt, kern)
             ab = algorithmic_bytes(npts, Bs * lanes, rs.rs_kernel_table_bytes(mesh, n, Bs, rsdt, kern))
-            sweep.append({"block": Bs, "kernel": rs.rs_kernel_name(mesh, n, Bs, rsdt, kern), "apply_ms": ms,
-                          "gflops": Bs * npts * flops_per_output(n) * (4 if is_c else 1) / ms / 1e6,
-                          "alg_gbs": ab / ms / 1e6, "frac_measured": ab / ms / 1e6 / peak,
+            row = traffic.get(f"config{cfg.index}_B{Bs}_n{n}_{kn}")
+            sweep.append({"block": Bs, "kernel": kn, "apply_ms": ms, "apply_ms_untuned": ms_untuned,
+                          "gflops": Bs * npts * flops_per_output(n) * conv / ms / 1e6,
+                          "gflops_executed": Bs * npts * flops_per_output(n) * lanes / ms / 1e6,
+                          "alg_gbs": ab / ms / 1e6, "frac_measured": ab / ms / 1e6 / peak, "frac_of_8TBs": ab / ms / 1e6 / 8000.0,
+                          "traffic": (int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])) if row else None,
                           "note": "block working set may fit L2" if 2 * b1.numel() * b1.element_size() < 126e6 else ""})
             del b1, b2
 
-    # ---- end to end through the host-buffer entry point ------------------------------------------
+    # ---- end to end through the host-buffer entry point (a7 workspace, created once) ---------------
     e2e = None
     if not args.no_e2e:
         del states, out, blk, hblk
         torch.cuda.empty_cache()
-        for _ in range(1):
-            rs.rs_hamiltonian_apply_states_host(mesh, n, coeffs, host_v, host_states, host_out, B)
+        ws = rs.rs_workspace_create(mesh, B, rsdt, npts)
+        rs.rs_hamiltonian_apply_states_stream(ws, n, coeffs, host_v, host_states, host_out)      # warm-up
         barrier()
         k = max(1, min(args.steps, 3))
         t = time.perf_counter()
         for _ in range(k):
-            rs.rs_hamiltonian_apply_states_host(mesh, n, coeffs, host_v, host_states, host_out, B)
+            rs.rs_hamiltonian_apply_states_stream(ws, n, coeffs, host_v, host_states, host_out)
         barrier()
         dt = (time.perf_counter() - t) / k
         if world > 1:
@@ -355,22 +412,43 @@ def main() -> None:
         sbytes = host_states.numel() * host_states.element_size()
         e2e = {"value": world * fl_step / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": sbytes + npts * 8,
                "d2h_bytes_per_step": sbytes, "ms_per_step": dt * 1e3, "steps": k,
-               "api": "rs_hamiltonian_apply_states_host (pinned host buffers)"}
+               "workspace_bytes": ws.nbytes,
+               "api": "rs_hamiltonian_apply_states_stream (pinned host buffers, 3-window workspace created once)"}
+        if rank == 0 and not args.no_cpu_baseline:
+            # the end-to-end OUTPUT is compared with the oracle on a seeded sample of orbitals (first / last block and two between)
+            import oracle
+            om = oracle.mesh_from_spheres(cfg.centers, cfg.radius, cfg.spacing)
+            assert om.npoints == npts
+            vc = synthetic.vloc_at(om.xyz(), cfg.centers, cfg.charges)
+            pick = sorted({0, nst - 1, *np.random.default_rng(12).integers(0, nst, 2).tolist()})
+            psi = np.stack([synthetic.orbital(cfg.seed, rank * nst + j, npts, is_c) for j in pick])
+            o = oracle.hpsi(om, n, oracle.fd_coeffs(n), vc, psi, nthreads=len(os.sched_getaffinity(0)))
+            g = np.empty_like(o)
+            g[:, rank_of] = host_out.numpy()[pick]
+            e2e["max_normwise_err"] = float(np.abs(g - o).max() / np.abs(o).max())
+            e2e["checked_orbitals"] = pick
+        del ws
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "c128" if is_c else "f64", "data": "synthetic",
-                "config": {**workload_config(cfg, n, B, npts), "kernel": kname, "parallelism": f"orbital-blocks x{world}",
-                           "mesh_build_s": t_mesh, "autotune_s": t_tune, "autotuned": not args.no_autotune, "nbricks": mesh.nbricks},
+                "config": {**workload_config(cfg, n, B, npts, nst), "kernel": kname, "parallelism": f"orbital-blocks x{world}",
+                           "mesh_build_s": t_mesh, "prepare_s": t_prepare, "autotune_s": t_tune, "autotuned": tune,
+                           "nbricks": mesh.nbricks},
+                "value_executed_flops": world * nst * npts * flops_per_output(n) * lanes / (ms_step * 1e-3) / 1e9,
+                "flop_convention": "BASELINE.json: nst*np*(2*(6n+1)+2), x4 for complex; *_executed counts the arithmetic "
+                                   "actually done (complex = 2 real lanes, reading S12)",
                 "roofline": roofline, "clocks": clocks, "gpu_launches": 3 * nblocks * args.steps}
+        if blocked:
+            line["blocked_resident"] = blocked
         if e2e:
             line["e2e"] = e2e
         if sweep:
             line["sweep"] = sweep
         if not args.no_cpu_baseline and world == 1:
             leg = cpu_oracle_leg(cfg, n, seconds_budget=15.0)
-            line["cpu_baseline"] = {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample")}
+            line["cpu_baseline"] = {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample", "one_core")}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -27,9 +27,14 @@
  *   - dtype RS_REAL64: element = double.  RS_COMPLEX128: element = interleaved (re, im) doubles; the
  *     weights and V are real, so a complex block of width B is computed as 2B independent real columns.
  *   - rs_block_pack / rs_block_unpack / rs_hamiltonian_apply are asynchronous on `stream`
- *     (a cudaStream_t passed as void*; NULL = legacy default stream), allocate nothing and never
- *     synchronise.  The first use of a given fd_order on a mesh uploads that order's neighbour table
- *     (one synchronous cudaMalloc + copy, then cached in the handle).
+ *     (a cudaStream_t passed as void*; NULL = legacy default stream).  After
+ *     rs_hamiltonian_prepare(mesh, fd_order, nst, dtype) they allocate nothing and never synchronise.
+ *     Without it, the first apply of a given (fd_order, block width) prepares lazily (host table build, one
+ *     synchronous cudaMalloc + copy, cached in the handle); blocks wider than 16 real columns also encode
+ *     their tensor maps once per psi buffer address (host-only work, cached).
+ *   - Alignment: vloc 8 bytes; states 8 (real) / 16 (complex) bytes; block buffers (psi, hpsi) 16 bytes
+ *     (bulk copies and vector accesses) -> RS_ERR_INVALID_ARG otherwise.
+ *   - A mesh handle is not thread-safe; the library keeps no global state.
  *   - Every function returns rs_status; nothing throws.  rs_last_error() gives thread-local text for
  *     the last non-OK status.  There is no CPU fallback: without a CUDA device the compute entry
  *     points return RS_ERR_CUDA.
@@ -120,8 +125,9 @@ rs_status rs_block_unpack(const rs_mesh *mesh, const void *block_dev, int block_
  * coeffs_host: c_0..c_n, dimensionless (the library forms w_k = -0.5 c_k / h^2 in fp64, reading S6).
  * vloc_dev: [np] doubles, mesh order.  psi_dev / hpsi_dev: block buffers of width nst (= the block
  * size B of this call: 1, 2, 4, ..., 64), distinct and non-overlapping.  Row np of hpsi is left as is.
- * Errors: NULL pointers, nst not a power of two in 1..64, fd_order < 1 or > max_fd_order, psi == hpsi
- * -> RS_ERR_INVALID_ARG; launch failure or no device -> RS_ERR_CUDA.                               */
+ * Errors: NULL pointers, nst not a power of two in 1..64, fd_order < 1 or > max_fd_order, psi and hpsi
+ * overlapping, psi / hpsi not 16-byte aligned, vloc not 8-byte aligned -> RS_ERR_INVALID_ARG; launch failure or
+ * no device -> RS_ERR_CUDA.                                                                         */
 rs_status rs_hamiltonian_apply(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
                                const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
                                rs_dtype dtype, void *stream);
@@ -130,21 +136,44 @@ rs_status rs_hamiltonian_apply_v(const rs_mesh *mesh, int fd_order, const double
                                  const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
                                  rs_dtype dtype, void *stream, rs_kernel kernel);
 
+/* Once per (mesh, fd_order, nst, dtype), before the first apply: build and upload the neighbour structure the chosen
+ * kernel needs (plain table for the gather kernel, per-plane records for the plane-sweep kernel).  May allocate and
+ * synchronise; afterwards rs_hamiltonian_apply for these arguments allocates nothing and never synchronises
+ * (SURVEY.md section 8(b) conventions).  Idempotent.                                                              */
+rs_status rs_hamiltonian_prepare(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype);
+
 /* Optional, once per (mesh, fd_order, nst, dtype): "measure, don't guess".  Runs the kernel a few times on the
  * caller's buffers (arguments as rs_hamiltonian_apply; hpsi receives H psi), reads back the clock each persistent
  * CTA recorded at the end of every plane, and deals the work to the CTAs again using the measured cost of every
  * (tile, plane) instead of the built-in cost model.  Later rs_hamiltonian_apply calls use the re-dealt tables; results
  * are unchanged up to rounding order.  SYNCHRONISES `stream` and replaces the mesh's device tables: no other call
  * on this mesh may be in flight on another stream or thread.  A call that only the gather kernel can serve is just
- * applied.  (The library keeps no global state besides the tuning knobs; a mesh handle is not thread-safe.)       */
+ * applied.                                                                                                        */
 rs_status rs_hamiltonian_autotune(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
                                   const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
                                   rs_dtype dtype, void *stream);
 
 /* ---- whole path on HOST buffers (step a7: the block sweep; used for the end-to-end number) --------
- * states_host / hstates_host: pinned or pageable host arrays [nst_total][ld] (ld >= np, mesh order);
- * vloc_host [np].  Uploads, then for each block of `block_size` orbitals: pack, apply, unpack; then
- * downloads H psi.  Allocates its device workspace per call and synchronises before returning.     */
+ * A workspace owns a ring of `nbuf` (2..8; 3 = upload / compute / download all overlapped) block-sized device
+ * windows, three streams and their events for blocks of `block_size` orbitals of `dtype` with leading dimension ld
+ * (>= np).  Device memory held: nbuf * 2 * (block_size*ld*elem + rs_block_bytes) + 8 np  (rs_workspace_bytes);
+ * it does not depend on the number of orbitals, so sets larger than the HBM stream through (BASELINE.json
+ * configs[4]: 1024 orbitals "processed in blocks ... streamed through HBM"; sec. IV).
+ * RS_ERR_ALLOC if the device memory cannot be had.                                                              */
+typedef struct rs_workspace rs_workspace; /* opaque */
+rs_status rs_workspace_create(const rs_mesh *mesh, int block_size, rs_dtype dtype, int64_t ld, int nbuf,
+                              rs_workspace **out);
+rs_status rs_workspace_destroy(rs_workspace *ws);
+size_t rs_workspace_bytes(const rs_workspace *ws);
+/* states_host / hstates_host: pinned (for overlap) or pageable host arrays [nst_total][ld], mesh order; vloc_host
+ * [np].  For each block of block_size orbitals: upload, pack, apply, unpack, download -- one cudaMemcpyAsync per
+ * block per direction, nothing allocated, pipelined over the ring.  Only the np points of every orbital are
+ * written to hstates_host (padding columns ld > np keep the caller's contents).  Returns after the last
+ * download has completed (synchronises its own three streams only).  The mesh must outlive the workspace.      */
+rs_status rs_hamiltonian_apply_states_stream(rs_workspace *ws, int fd_order, const double *coeffs_host,
+                                             const double *vloc_host, const void *states_host, void *hstates_host,
+                                             int nst_total);
+/* Convenience form of the same: creates a 3-window workspace, streams, destroys it (allocation per call).      */
 rs_status rs_hamiltonian_apply_states_host(const rs_mesh *mesh, int fd_order, const double *coeffs_host,
                                            const double *vloc_host, const void *states_host,
                                            void *hstates_host, int64_t ld, int nst_total, int block_size,
@@ -156,15 +185,20 @@ const char *rs_kernel_name(const rs_mesh *mesh, int fd_order, int nst, rs_dtype 
 /* Bytes of neighbour structure the chosen kernel reads per call (for the roofline's algorithmic bytes). */
 int64_t rs_kernel_table_bytes(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, rs_kernel kernel);
 int rs_version(void);
-/* Tuning knobs for tests and ablations (not needed for normal use); they take effect for tables built
- * afterwards.  "sweep_planes": x-slab thickness of a plane-sweep work item (default 32), "sweep_planes_tuned": the same
- * after rs_hamiltonian_autotune (default: the whole x extent); "sweep_ctas":
- * number of persistent CTAs (0 = one per SM); "sweep_tensor": 1 = use the 2-D tensor-map copies also for
- * 16-column blocks; "sweep_shape": 1 = run fd_order 4 on the experimental 12-warp kernel shape; "sweep_min_split": fewest
- * output planes of a work piece cut off when dealing (default 3); "sweep_tune_rounds": measure / re-deal rounds of
- * rs_hamiltonian_autotune (default 3).
- * Unknown name -> RS_ERR_INVALID_ARG.                                                                  */
-rs_status rs_set_tuning(const char *name, int value);
+/* Options of the plane-sweep kernel's host-side work dealing, PER MESH (no process-global state).  Defaults:
+ * rs_sweep_options_default().  rs_mesh_set_sweep_options() drops the tables (and measured costs) built so far, so
+ * the next prepare / apply builds them under the new options; it synchronises the device.  For tests and ablations;
+ * normal use never needs it (the block size is the only run-time knob of the method).               */
+typedef struct {
+    int planes;        /* x-slab thickness of a work item while the step costs are modelled (default 32)            */
+    int planes_tuned;  /* the same once rs_hamiltonian_autotune measured them (default 1 << 20: whole tile columns)  */
+    int ctas;          /* persistent CTAs (0 = one per SM)                                                          */
+    int force_tensor;  /* 1 = use the 2-D tensor-map copies also for 16-column blocks                               */
+    int min_split;     /* fewest output planes of a work piece cut off when dealing (default 3)                     */
+    int tune_rounds;   /* measure / re-deal rounds of rs_hamiltonian_autotune (default 3)                           */
+} rs_sweep_options;
+rs_status rs_sweep_options_default(rs_sweep_options *out);
+rs_status rs_mesh_set_sweep_options(rs_mesh *mesh, const rs_sweep_options *opt);
 /* Host-only diagnostic (no device needed): build the plane-sweep kernel's compact records for (mesh,
  * fd_order, block width nst of dtype) dealt to `nctas` CTAs with slabs of `max_planes`, replay them
  * symbolically and verify that they expand to exactly the plain table of rs_mesh_get_index_map and that
@@ -177,9 +211,9 @@ rs_status rs_sweep_selfcheck(const rs_mesh *mesh, int fd_order, int nst, rs_dtyp
                              int64_t *stats_host);
 
 /* Per-CTA figures of the plane-sweep kernel's last launch for (mesh, fd_order, nst, dtype), for calibrating
- * the cost model that deals work to the persistent CTAs: out_host [max_ctas][5] = {clock ticks spent, steps,
- * work pieces, modelled load x1000, full warp-steps}.  Synchronises the device.  Returns the number of
- * CTAs written (0 if that kernel has not run).                                                           */
+ * the cost model that deals work to the persistent CTAs: out_host [max_ctas][5] = {clock ticks spent in the last
+ * MEASURING launch (rs_hamiltonian_autotune; production launches record nothing), steps, work pieces, modelled
+ * load x1000, full warp-steps}.  Synchronises the device.  Returns the number of CTAs written (0 if no tables).  */
 int64_t rs_sweep_stats(const rs_mesh *mesh, int fd_order, int nst, rs_dtype dtype, int64_t *out_host, int64_t max_ctas);
 
 #ifdef __cplusplus

@@ -35,9 +35,17 @@ EXPORTS = (
     "rs_mesh_create", "rs_mesh_create_ordered", "rs_mesh_create_box", "rs_mesh_destroy", "rs_mesh_npoints",
     "rs_mesh_spacing", "rs_mesh_nbricks", "rs_mesh_get_points", "rs_mesh_get_index_map", "rs_block_bytes",
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
-    "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version", "rs_set_tuning",
+    "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version",
+    "rs_sweep_options_default", "rs_mesh_set_sweep_options", "rs_hamiltonian_prepare",
+    "rs_workspace_create", "rs_workspace_destroy", "rs_workspace_bytes", "rs_hamiltonian_apply_states_stream",
     "rs_sweep_selfcheck", "rs_sweep_stats", "rs_hamiltonian_autotune",
 )
+
+
+class SweepOptions(C.Structure):
+    """rs_sweep_options of include/rs.h (per-mesh options of the plane-sweep kernel's work dealing)."""
+    _fields_ = [("planes", C.c_int), ("planes_tuned", C.c_int), ("ctas", C.c_int), ("force_tensor", C.c_int),
+                ("min_split", C.c_int), ("tune_rounds", C.c_int)]
 
 
 class RsError(RuntimeError):
@@ -75,13 +83,20 @@ def _load() -> C.CDLL:
     L.rs_hamiltonian_autotune.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp]
     L.rs_hamiltonian_apply_v.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp, C.c_int]
     L.rs_hamiltonian_apply_states_host.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int]
+    L.rs_workspace_create.argtypes = [vp, C.c_int, C.c_int, C.c_int64, C.c_int, C.POINTER(vp)]
+    L.rs_workspace_destroy.argtypes = [vp]
+    L.rs_workspace_bytes.argtypes = [vp]
+    L.rs_workspace_bytes.restype = C.c_size_t
+    L.rs_hamiltonian_apply_states_stream.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int]
     L.rs_last_error.restype = C.c_char_p
     L.rs_kernel_name.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
     L.rs_kernel_name.restype = C.c_char_p
     L.rs_kernel_table_bytes.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
     L.rs_kernel_table_bytes.restype = C.c_int64
     L.rs_version.restype = C.c_int
-    L.rs_set_tuning.argtypes = [C.c_char_p, C.c_int]
+    L.rs_sweep_options_default.argtypes = [C.POINTER(SweepOptions)]
+    L.rs_mesh_set_sweep_options.argtypes = [vp, C.POINTER(SweepOptions)]
+    L.rs_hamiltonian_prepare.argtypes = [vp, C.c_int, C.c_int, C.c_int]
     L.rs_sweep_stats.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64), C.c_int64]
     L.rs_sweep_stats.restype = C.c_int64
     L.rs_sweep_selfcheck.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]
@@ -168,8 +183,25 @@ def rs_version() -> int:
     return int(_lib.rs_version())
 
 
-def rs_set_tuning(name: str, value: int) -> None:
-    _check(_lib.rs_set_tuning(name.encode(), value))
+def rs_sweep_options_default() -> SweepOptions:
+    o = SweepOptions()
+    _check(_lib.rs_sweep_options_default(C.byref(o)))
+    return o
+
+
+def rs_mesh_set_sweep_options(mesh, options: SweepOptions | None = None, **fields) -> None:
+    """Set the mesh's plane-sweep options (defaults, overridden by `fields`); tables built so far are dropped."""
+    o = options if options is not None else rs_sweep_options_default()
+    for k, v in fields.items():
+        if k not in dict(SweepOptions._fields_):
+            raise RsError(RS_ERR_INVALID_ARG, f"unknown sweep option {k}")
+        setattr(o, k, int(v))
+    _check(_lib.rs_mesh_set_sweep_options(mesh.handle, C.byref(o)))
+
+
+def rs_hamiltonian_prepare(mesh, fd_order: int, nst: int, dtype: int = RS_REAL64) -> None:
+    """Build and upload the neighbour structure for (fd_order, nst, dtype) now; later applies allocate nothing."""
+    _check(_lib.rs_hamiltonian_prepare(mesh.handle, fd_order, nst, dtype))
 
 
 def rs_sweep_stats(mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, max_ctas: int = 4096) -> np.ndarray:
@@ -274,6 +306,38 @@ def rs_hamiltonian_apply_states_host(mesh: Mesh, fd_order: int, coeffs, vloc_hos
     _check(_lib.rs_hamiltonian_apply_states_host(mesh.handle, fd_order, _dptr(c), _ptr(vloc_host), _ptr(states_host),
                                                  _ptr(hstates_host), ld, nst_total, block_size,
                                                  _dtype_of(states_host)))
+
+
+class Workspace:
+    """Owner of an rs_workspace handle (ring of block-sized device windows + streams); keeps its mesh alive."""
+
+    def __init__(self, mesh: Mesh, block_size: int, dtype: int, ld: int, nbuf: int = 3):
+        out = C.c_void_p()
+        _check(_lib.rs_workspace_create(mesh.handle, block_size, dtype, ld, nbuf, C.byref(out)))
+        self._h, self.mesh, self.block_size, self.dtype, self.ld = out, mesh, block_size, dtype, ld
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h and _lib is not None:
+            _lib.rs_workspace_destroy(h)
+
+    @property
+    def nbytes(self) -> int:
+        return int(_lib.rs_workspace_bytes(self._h))
+
+
+def rs_workspace_create(mesh: Mesh, block_size: int, dtype: int, ld: int, nbuf: int = 3) -> Workspace:
+    return Workspace(mesh, block_size, dtype, ld, nbuf)
+
+
+def rs_hamiltonian_apply_states_stream(ws: Workspace, fd_order: int, coeffs, vloc_host, states_host, hstates_host) -> None:
+    """Whole path on HOST arrays [nst_total][ld] through a workspace created once (no allocation per call)."""
+    c = np.ascontiguousarray(coeffs, dtype=np.float64)
+    nst_total, ld = int(states_host.shape[0]), int(states_host.shape[1])
+    if ld != ws.ld or _dtype_of(states_host) != ws.dtype:
+        raise RsError(RS_ERR_INVALID_ARG, "states do not match the workspace (leading dimension / dtype)")
+    _check(_lib.rs_hamiltonian_apply_states_stream(ws._h, fd_order, _dptr(c), _ptr(vloc_host), _ptr(states_host),
+                                                   _ptr(hstates_host), nst_total))
 
 
 def rs_kernel_name(mesh: Mesh, fd_order: int, nst: int, dtype: int = RS_REAL64, kernel: int = RS_KERNEL_AUTO) -> str:

@@ -1,5 +1,6 @@
 // C-ABI entry points: argument checks, weight formation, kernel dispatch, host-buffer sweep.
 #include <cstring>
+#include <new>
 #include <vector>
 
 #include "rs_internal.h"
@@ -37,6 +38,10 @@ static rs_status check_apply(const rs_mesh *m, int n, const double *coeffs, cons
     const char *a = (const char *)psi, *b = (const char *)hpsi;
     if (a == b || (a < b + bytes && b < a + bytes))
         return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: psi and hpsi overlap");
+    // bulk copies (cp.async.bulk, tensor maps) and the 16-byte vector accesses of the gather kernel
+    if ((((uintptr_t)psi | (uintptr_t)hpsi) & 15u) != 0)
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: psi and hpsi must be 16-byte aligned");
+    if (((uintptr_t)vloc & 7u) != 0) return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply: vloc must be 8-byte aligned");
     return RS_OK;
 }
 
@@ -108,7 +113,159 @@ extern "C" int64_t rs_kernel_table_bytes(const rs_mesh *m, int n, int nst, rs_dt
     return m->np * 6 * (int64_t)n * 4;
 }
 
-// Whole path on host buffers (a7): H2D, then per block pack -> apply -> unpack, then D2H.
+// ---------------------------------------------------------------------------------------------
+// Block sweep on HOST buffers (a7): a streaming driver.  A workspace owns a ring of `nbuf` block-sized device
+// windows (states slab in, block, H block, states slab out), three streams and the events that order them;
+// block k uses window k mod nbuf: upload of block k + 1, compute of block k and download of block k - 1 overlap
+// (PCIe is full duplex).  Nothing is allocated per call and the device never holds more than nbuf blocks, so an
+// orbital set larger than the HBM streams through (BASELINE.json configs[4]; sec. IV: block size vs memory).
+// ---------------------------------------------------------------------------------------------
+struct rs_workspace {
+    const rs_mesh *m = nullptr;
+    int B = 0, nbuf = 0;
+    rs_dtype dtype = RS_REAL64;
+    int64_t ld = 0;
+    size_t esz = 8, slab = 0, bbytes = 0;
+    std::vector<void *> d_in, d_out, d_psi, d_hpsi;
+    double *d_v = nullptr;
+    cudaStream_t s_in = nullptr, s_cmp = nullptr, s_out = nullptr;
+    std::vector<cudaEvent_t> ev_in, ev_cmp, ev_out;
+    cudaEvent_t ev_v = nullptr;
+};
+
+extern "C" rs_status rs_workspace_destroy(rs_workspace *ws)
+{
+    if (!ws) return RS_OK;
+    if (ws->s_in) cudaStreamSynchronize(ws->s_in);
+    if (ws->s_cmp) cudaStreamSynchronize(ws->s_cmp);
+    if (ws->s_out) cudaStreamSynchronize(ws->s_out);
+    for (auto *v : {&ws->d_in, &ws->d_out, &ws->d_psi, &ws->d_hpsi})
+        for (void *p : *v) cudaFree(p);
+    cudaFree(ws->d_v);
+    for (auto *v : {&ws->ev_in, &ws->ev_cmp, &ws->ev_out})
+        for (cudaEvent_t e : *v)
+            if (e) cudaEventDestroy(e);
+    if (ws->ev_v) cudaEventDestroy(ws->ev_v);
+    if (ws->s_in) cudaStreamDestroy(ws->s_in);
+    if (ws->s_cmp) cudaStreamDestroy(ws->s_cmp);
+    if (ws->s_out) cudaStreamDestroy(ws->s_out);
+    delete ws;
+    return RS_OK;
+}
+
+extern "C" rs_status rs_workspace_create(const rs_mesh *m, int B, rs_dtype dtype, int64_t ld, int nbuf, rs_workspace **out)
+{
+    if (!m || !out || !pow2_in(B, 1, RS_MAX_BLOCK) || (dtype != RS_REAL64 && dtype != RS_COMPLEX128) || ld < m->np || nbuf < 2 || nbuf > 8)
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_workspace_create: bad argument");
+    *out = nullptr;
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    rs_workspace *ws = new (std::nothrow) rs_workspace;
+    if (!ws) return rs_fail(RS_ERR_ALLOC, "out of host memory");
+    ws->m = m, ws->B = B, ws->nbuf = nbuf, ws->dtype = dtype, ws->ld = ld;
+    ws->esz = dtype == RS_COMPLEX128 ? 16 : 8;
+    ws->slab = (size_t)B * ld * ws->esz;
+    ws->bbytes = rs_block_bytes(m, B, dtype);
+#define WS_TRY(call)                                                                               \
+    do {                                                                                           \
+        cudaError_t _e = (call);                                                                   \
+        if (_e != cudaSuccess) {                                                                   \
+            rs_workspace_destroy(ws);                                                              \
+            return rs_fail(_e == cudaErrorMemoryAllocation ? RS_ERR_ALLOC : RS_ERR_CUDA,           \
+                           std::string(#call) + ": " + cudaGetErrorString(_e));                    \
+        }                                                                                          \
+    } while (0)
+    WS_TRY(cudaStreamCreateWithFlags(&ws->s_in, cudaStreamNonBlocking));
+    WS_TRY(cudaStreamCreateWithFlags(&ws->s_cmp, cudaStreamNonBlocking));
+    WS_TRY(cudaStreamCreateWithFlags(&ws->s_out, cudaStreamNonBlocking));
+    WS_TRY(cudaEventCreateWithFlags(&ws->ev_v, cudaEventDisableTiming));
+    WS_TRY(cudaMalloc(&ws->d_v, (size_t)m->np * 8));
+    for (int q = 0; q < nbuf; ++q) {
+        void *p = nullptr;
+        cudaEvent_t e = nullptr;
+        WS_TRY(cudaMalloc(&p, ws->slab));
+        ws->d_in.push_back(p);
+        WS_TRY(cudaMalloc(&p, ws->slab));
+        ws->d_out.push_back(p);
+        WS_TRY(cudaMalloc(&p, ws->bbytes));
+        ws->d_psi.push_back(p);
+        WS_TRY(cudaMalloc(&p, ws->bbytes));
+        ws->d_hpsi.push_back(p);
+        WS_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ws->ev_in.push_back(e);
+        WS_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ws->ev_cmp.push_back(e);
+        WS_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ws->ev_out.push_back(e);
+    }
+#undef WS_TRY
+    *out = ws;
+    return RS_OK;
+}
+
+extern "C" size_t rs_workspace_bytes(const rs_workspace *ws)
+{
+    return ws ? (size_t)ws->nbuf * 2 * (ws->slab + ws->bbytes) + (size_t)ws->m->np * 8 : 0;
+}
+
+extern "C" rs_status rs_hamiltonian_apply_states_stream(rs_workspace *ws, int n, const double *coeffs, const double *vloc_host,
+                                                        const void *states_host, void *hstates_host, int nst_total)
+{
+    if (!ws || !coeffs || !vloc_host || !states_host || !hstates_host || nst_total < 1 || n < 1 || n > ws->m->max_n)
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply_states_stream: bad argument");
+    const rs_mesh *m = ws->m;
+    const int B = ws->B, nblocks = (nst_total + B - 1) / B;
+    const size_t esz = ws->esz, row = (size_t)m->np * esz, pitch = (size_t)ws->ld * esz;
+    rs_status rc = rs_hamiltonian_prepare(m, n, B, ws->dtype);   // tables now, not inside the block loop
+    if (rc != RS_OK) return rc;
+#define WS_TRY(call)                                                                               \
+    do {                                                                                           \
+        cudaError_t _e = (call);                                                                   \
+        if (_e != cudaSuccess) {                                                                   \
+            cudaDeviceSynchronize();                                                               \
+            return rs_fail(RS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e));       \
+        }                                                                                          \
+    } while (0)
+    WS_TRY(cudaMemcpyAsync(ws->d_v, vloc_host, (size_t)m->np * 8, cudaMemcpyHostToDevice, ws->s_in));
+    WS_TRY(cudaEventRecord(ws->ev_v, ws->s_in));
+    WS_TRY(cudaStreamWaitEvent(ws->s_cmp, ws->ev_v, 0));
+    for (int k = 0; k < nblocks; ++k) {
+        const int w = k % ws->nbuf, ist0 = k * B, nb = nst_total - ist0 < B ? nst_total - ist0 : B;
+        const char *src = (const char *)states_host + (size_t)ist0 * pitch;
+        char *dst = (char *)hstates_host + (size_t)ist0 * pitch;
+        // upload: the window's previous pack (block k - nbuf) must have read its slab
+        if (k >= ws->nbuf) WS_TRY(cudaStreamWaitEvent(ws->s_in, ws->ev_cmp[w], 0));
+        if (pitch == row)
+            WS_TRY(cudaMemcpyAsync(ws->d_in[w], src, (size_t)nb * row, cudaMemcpyHostToDevice, ws->s_in));
+        else   // padded leading dimension: only the np points of every orbital travel
+            WS_TRY(cudaMemcpy2DAsync(ws->d_in[w], pitch, src, pitch, row, nb, cudaMemcpyHostToDevice, ws->s_in));
+        WS_TRY(cudaEventRecord(ws->ev_in[w], ws->s_in));
+        // compute: after the upload, and after the window's previous download (block k - nbuf) left d_out
+        WS_TRY(cudaStreamWaitEvent(ws->s_cmp, ws->ev_in[w], 0));
+        if (k >= ws->nbuf) WS_TRY(cudaStreamWaitEvent(ws->s_cmp, ws->ev_out[w], 0));
+        rc = rs_block_pack(m, ws->d_in[w], ws->ld, 0, nb, B, ws->d_psi[w], ws->dtype, ws->s_cmp);
+        if (rc == RS_OK) rc = rs_hamiltonian_apply(m, n, coeffs, ws->d_v, ws->d_psi[w], ws->d_hpsi[w], B, ws->dtype, ws->s_cmp);
+        if (rc == RS_OK) rc = rs_block_unpack(m, ws->d_hpsi[w], B, nb, ws->d_out[w], ws->ld, 0, ws->dtype, ws->s_cmp);
+        if (rc != RS_OK) {
+            cudaDeviceSynchronize();
+            return rc;
+        }
+        WS_TRY(cudaEventRecord(ws->ev_cmp[w], ws->s_cmp));
+        // download: unpack never writes beyond np, so only [0, np) of every row goes back (the caller's padding is untouched)
+        WS_TRY(cudaStreamWaitEvent(ws->s_out, ws->ev_cmp[w], 0));
+        if (pitch == row)
+            WS_TRY(cudaMemcpyAsync(dst, ws->d_out[w], (size_t)nb * row, cudaMemcpyDeviceToHost, ws->s_out));
+        else
+            WS_TRY(cudaMemcpy2DAsync(dst, pitch, ws->d_out[w], pitch, row, nb, cudaMemcpyDeviceToHost, ws->s_out));
+        WS_TRY(cudaEventRecord(ws->ev_out[w], ws->s_out));
+    }
+    WS_TRY(cudaStreamSynchronize(ws->s_out));
+    WS_TRY(cudaStreamSynchronize(ws->s_cmp));
+    WS_TRY(cudaStreamSynchronize(ws->s_in));
+#undef WS_TRY
+    return RS_OK;
+}
+
+// Convenience form: a temporary 3-window workspace per call (allocation inside; use the workspace form in a loop).
 extern "C" rs_status rs_hamiltonian_apply_states_host(const rs_mesh *m, int n, const double *coeffs,
                                                       const double *vloc_host, const void *states_host,
                                                       void *hstates_host, int64_t ld, int nst_total, int B,
@@ -118,114 +275,45 @@ extern "C" rs_status rs_hamiltonian_apply_states_host(const rs_mesh *m, int n, c
         !pow2_in(B, 1, RS_MAX_BLOCK) || n < 1 || n > m->max_n || (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
         return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply_states_host: bad argument");
     if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
-    const size_t esz = dtype == RS_COMPLEX128 ? 16 : 8;
-    const size_t sbytes = (size_t)nst_total * ld * esz, bbytes = rs_block_bytes(m, B, dtype);
-    // Three streams: upload of block k + 1, compute of block k and download of block k - 1 overlap (PCIe is full duplex);
-    // two pairs of block buffers so that compute never waits for its own previous unpack to drain.
-    void *d_states = nullptr, *d_out = nullptr, *d_psi[2] = {nullptr, nullptr}, *d_hpsi[2] = {nullptr, nullptr};
-    double *d_v = nullptr;
-    cudaStream_t s_in = nullptr, s_cmp = nullptr, s_out = nullptr;
-    const int nblocks = (nst_total + B - 1) / B;
-    std::vector<cudaEvent_t> ev_in(nblocks, nullptr), ev_cmp(nblocks, nullptr);
-    rs_status rc = RS_OK;
-    auto cleanup = [&]() {
-        cudaFree(d_states), cudaFree(d_out), cudaFree(d_psi[0]), cudaFree(d_psi[1]), cudaFree(d_hpsi[0]), cudaFree(d_hpsi[1]), cudaFree(d_v);
-        for (cudaEvent_t e : ev_in)
-            if (e) cudaEventDestroy(e);
-        for (cudaEvent_t e : ev_cmp)
-            if (e) cudaEventDestroy(e);
-        if (s_in) cudaStreamDestroy(s_in);
-        if (s_cmp) cudaStreamDestroy(s_cmp);
-        if (s_out) cudaStreamDestroy(s_out);
-    };
-#define TRY_OR_CLEAN(call)                                                                     \
-    do {                                                                                       \
-        cudaError_t _e = (call);                                                               \
-        if (_e != cudaSuccess) {                                                               \
-            cudaDeviceSynchronize();                                                           \
-            cleanup();                                                                         \
-            return rs_fail(RS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e));   \
-        }                                                                                      \
-    } while (0)
-    TRY_OR_CLEAN(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
-    TRY_OR_CLEAN(cudaStreamCreateWithFlags(&s_cmp, cudaStreamNonBlocking));
-    TRY_OR_CLEAN(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
-    TRY_OR_CLEAN(cudaMalloc(&d_states, sbytes));
-    TRY_OR_CLEAN(cudaMalloc(&d_out, sbytes));
-    for (int q = 0; q < 2; ++q) {
-        TRY_OR_CLEAN(cudaMalloc(&d_psi[q], bbytes));
-        TRY_OR_CLEAN(cudaMalloc(&d_hpsi[q], bbytes));
-    }
-    TRY_OR_CLEAN(cudaMalloc(&d_v, (size_t)m->np * 8));
-    TRY_OR_CLEAN(cudaMemcpyAsync(d_v, vloc_host, (size_t)m->np * 8, cudaMemcpyHostToDevice, s_in));
-    for (int k = 0; k < nblocks; ++k) {
-        const int ist0 = k * B, nb = nst_total - ist0 < B ? nst_total - ist0 : B;
-        const size_t off = (size_t)ist0 * ld * esz, bytes = (size_t)nb * ld * esz;
-        TRY_OR_CLEAN(cudaEventCreateWithFlags(&ev_in[k], cudaEventDisableTiming));
-        TRY_OR_CLEAN(cudaEventCreateWithFlags(&ev_cmp[k], cudaEventDisableTiming));
-        TRY_OR_CLEAN(cudaMemcpyAsync((char *)d_states + off, (const char *)states_host + off, bytes, cudaMemcpyHostToDevice, s_in));
-        TRY_OR_CLEAN(cudaEventRecord(ev_in[k], s_in));
-        TRY_OR_CLEAN(cudaStreamWaitEvent(s_cmp, ev_in[k], 0));
-        rc = rs_block_pack(m, d_states, ld, ist0, nb, B, d_psi[k & 1], dtype, s_cmp);
-        if (rc == RS_OK) rc = rs_hamiltonian_apply(m, n, coeffs, d_v, d_psi[k & 1], d_hpsi[k & 1], B, dtype, s_cmp);
-        if (rc == RS_OK) rc = rs_block_unpack(m, d_hpsi[k & 1], B, nb, d_out, ld, ist0, dtype, s_cmp);
-        if (rc != RS_OK) {
-            cudaDeviceSynchronize();
-            cleanup();
-            return rc;
-        }
-        TRY_OR_CLEAN(cudaEventRecord(ev_cmp[k], s_cmp));
-        TRY_OR_CLEAN(cudaStreamWaitEvent(s_out, ev_cmp[k], 0));
-        TRY_OR_CLEAN(cudaMemcpyAsync((char *)hstates_host + off, (const char *)d_out + off, bytes, cudaMemcpyDeviceToHost, s_out));
-    }
-    TRY_OR_CLEAN(cudaStreamSynchronize(s_out));
-    TRY_OR_CLEAN(cudaStreamSynchronize(s_cmp));
-    TRY_OR_CLEAN(cudaStreamSynchronize(s_in));
-    cleanup();
-#undef TRY_OR_CLEAN
+    rs_workspace *ws = nullptr;
+    rs_status rc = rs_workspace_create(m, B, dtype, ld, 3, &ws);
+    if (rc != RS_OK) return rc;
+    rc = rs_hamiltonian_apply_states_stream(ws, n, coeffs, vloc_host, states_host, hstates_host, nst_total);
+    rs_workspace_destroy(ws);
+    return rc;
+}
+
+std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, int64_t *stats);
+
+extern "C" rs_status rs_sweep_options_default(rs_sweep_options *out)
+{
+    if (!out) return rs_fail(RS_ERR_INVALID_ARG, "rs_sweep_options_default: null argument");
+    *out = rs_mesh().opt;
     return RS_OK;
 }
 
-void rs_sweep_set_max_planes(int v);
-void rs_sweep_set_force_tensor(int v);
-void rs_sweep_set_nctas(int v);
-void rs_sweep_set_shape(int v);
-void rs_sweep_set_tuned_planes(int v);
-void rs_sweep_set_min_split(int v);
-void rs_sweep_set_tune_rounds(int v);
-std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, int64_t *stats);
-
-extern "C" rs_status rs_set_tuning(const char *name, int value)
+extern "C" rs_status rs_mesh_set_sweep_options(rs_mesh *m, const rs_sweep_options *opt)
 {
-    if (name && std::strcmp(name, "sweep_planes") == 0) {
-        rs_sweep_set_max_planes(value);
-        return RS_OK;
+    if (!m || !opt || opt->planes < 1 || opt->planes_tuned < 1 || opt->ctas < 0 || opt->min_split < 1 || opt->tune_rounds < 1)
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_mesh_set_sweep_options: bad argument");
+    if (m->have_device) {
+        RS_CUDA_TRY(cudaDeviceSynchronize());   // no launch may still read the tables that are dropped
+        rs_sweep_free(m);
     }
-    if (name && std::strcmp(name, "sweep_tensor") == 0) {
-        rs_sweep_set_force_tensor(value);
-        return RS_OK;
-    }
-    if (name && std::strcmp(name, "sweep_planes_tuned") == 0) {
-        rs_sweep_set_tuned_planes(value);
-        return RS_OK;
-    }
-    if (name && std::strcmp(name, "sweep_min_split") == 0) {
-        rs_sweep_set_min_split(value);
-        return RS_OK;
-    }
-    if (name && std::strcmp(name, "sweep_tune_rounds") == 0) {
-        rs_sweep_set_tune_rounds(value);
-        return RS_OK;
-    }
-    if (name && std::strcmp(name, "sweep_shape") == 0) {
-        rs_sweep_set_shape(value);
-        return RS_OK;
-    }
-    if (name && std::strcmp(name, "sweep_ctas") == 0) {
-        rs_sweep_set_nctas(value);
-        return RS_OK;
-    }
-    return rs_fail(RS_ERR_INVALID_ARG, "rs_set_tuning: unknown knob");
+    m->sweep_costs.clear();
+    m->opt = *opt;
+    return RS_OK;
+}
+
+extern "C" rs_status rs_hamiltonian_prepare(const rs_mesh *m, int n, int nst, rs_dtype dtype)
+{
+    if (!m || n < 1 || n > m->max_n || !pow2_in(nst, 1, RS_MAX_BLOCK) || (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_prepare: bad argument");
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
+    if (resolve_kernel(m, n, ncol, RS_KERNEL_AUTO) == RS_KERNEL_SWEEP) return rs_sweep_prepare(m, n, ncol);
+    const int32_t *d_map = nullptr;
+    return rs_mesh_device_map(m, n, &d_map);
 }
 
 int64_t rs_sweep_read_stats(const rs_mesh *cm, int n, int ncol, int64_t *out, int64_t max_ctas);

@@ -59,6 +59,13 @@ struct rs_sweep_tables {
     std::vector<int64_t> host_stats;                 // per CTA: {steps, pieces, modelled load x 1000, full warp-steps}
 };
 
+// encoded tensor maps of one psi buffer (rs_sweep.cu: 6 CUtensorMap of 128 bytes), kept per (pointer, row pitch)
+struct rs_sweep_map_cache {
+    const double *psi = nullptr;
+    int ncol = 0;
+    alignas(64) unsigned char bytes[6 * 128];
+};
+
 struct rs_mesh {
     int64_t np = 0;
     double h = 0.0;
@@ -81,6 +88,8 @@ struct rs_mesh {
     int32_t *d_map[RS_MAX_FD_ORDER + 1] = {nullptr};                 // [np][6n], built lazily per order
     std::map<std::pair<int, int>, rs_sweep_tables> sweep;            // (fd_order, ncol) -> tables, built lazily
     std::map<std::pair<int, int>, rs_sweep_costs> sweep_costs;       // measured step costs, if autotuned
+    std::vector<rs_sweep_map_cache> map_cache;                       // tensor maps per psi buffer (blocks wider than 16 columns)
+    rs_sweep_options opt = {32, 1 << 20, 0, 0, 3, 3};                // rs_mesh_set_sweep_options
 };
 
 void rs_set_error(const std::string &msg);
@@ -123,5 +132,6 @@ void rs_sweep_free(rs_mesh *m);
 // host-only construction of the records; false if a plane needs more than RS_SWEEP_MAXRUN runs
 bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out,
                          const rs_sweep_costs *measured = nullptr);
+rs_status rs_sweep_prepare(const rs_mesh *m, int n, int ncol);   // build + upload the tables now
 rs_status rs_sweep_autotune(const rs_mesh *m, int n, const rs_weights &w, const double *vloc, const double *psi, double *hpsi,
                             int ncol, cudaStream_t st);

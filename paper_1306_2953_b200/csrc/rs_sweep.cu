@@ -60,9 +60,8 @@ constexpr int SW_NBOX = 6;               // tensor-map box heights 1, 2, 4, 8, 1
 
 // Kernel shape: star half-width N, tile of TY x 16 (y, z) points, register patch of PY x 4 points per thread,
 // NGROUPS producer groups of 4 warps.  Compiled shapes (rs_sweep_variant()):
-//   <4, 16, 4, 2>  the default for fd_order 4: 8 consumer warps, 16 outputs per thread, 4 pending planes in registers
+//   <4, 16, 4, 2>  fd_order 4: 8 consumer warps, 16 outputs per thread, 4 pending planes in registers
 //   <6,  8, 2, 2>  fd_order 6: 6 pending planes of a 4 x 4 patch do not fit the register file; 2 x 4 patches do
-//   <4, 12, 2, 1>  experiment for fd_order 4: 12 lighter consumer warps (rs_set_tuning("sweep_shape", 1))
 template <int N_, int TY_, int PY_, int NGROUPS_>
 struct sweep_shape {
     static constexpr int N = N_, TY = TY_, PY = PY_, NGROUPS = NGROUPS_;
@@ -90,7 +89,6 @@ struct sweep_shape {
 };
 using shape_n4 = sweep_shape<4, 16, 4, 2>;
 using shape_n6 = sweep_shape<6, 8, 2, 2>;
-using shape_n4w12 = sweep_shape<4, 12, 2, 1>;
 
 // the same numbers at run time, for the host-side builder
 struct shape_rt {
@@ -234,17 +232,6 @@ struct sweep_maps {
     CUtensorMap box[SW_NBOX];    // psi as a [np+1][ncol] fp64 tensor, box {16, 1|2|4|8|16|24}
 };
 
-// Optional timeline of one CTA (development builds only, -DSW_TRACE): clock64 stamps per step after the per-CTA ticks.
-#ifndef SW_EXP
-#define SW_EXP 0   // development builds: bit 0 drops the FULL-mode stores, bit 1 the tensor-memory traffic, bit 2 the z/y loads,
-                   // bit 3 stamps the producer instead of the consumer, bit 6 makes the consumers only wait and release
-#endif
-#ifdef SW_TRACE
-#define SW_STAMP(cond, t, k) do { if ((cond) && blockIdx.x == SW_TRACE && (t) < 256) a.cycles[gridDim.x + (t) * 8 + (k)] = clock64(); } while (0)
-#else
-#define SW_STAMP(cond, t, k) do { } while (0)
-#endif
-
 // ---- producer warps: NGROUPS groups of 4 warps stage plane after plane, group g taking steps t = g (mod NGROUPS) ----
 // Inside a group every warp takes a quarter of each job (copy runs, zero fill, V / offset staging) and arrives
 // once on the stage's "full" barrier.  Two groups because a step's chain of barrier waits, copy issues and
@@ -307,7 +294,6 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         fetch_v(rs);
     }
     for (int t = group; t < nsteps; t += G) {
-        SW_STAMP(gtid == 0, t, 0);
         // everything the copies need is read from the record (present: fetch_v waited for it) BEFORE the wait for
         // the stage, so that the copies leave right after the consumers release it
         const unsigned char *rp = ring + (size_t)rs * S::REC_BYTES;
@@ -319,7 +305,6 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         if (lane < SW_MAXRUN / 4) run = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
         const uint32_t len = run.y >> 16, slot = run.y & 0xffffu;
         mbar_wait(empty0 + 8u * stage, eparity);
-        SW_STAMP(gtid == 0, t, 1);
         fence_proxy_async();   // earlier generic accesses to this stage and to the record slot reused below (ordered before us by the barrier) before our async copies
         // ---- copy runs --------------------------------------------------------------------------------
         if (len) {
@@ -335,7 +320,6 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
             }
         }
         if (gtid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
-        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 4);
         // ---- zero fill: bit s of the record's bitmap says that slot s of the [WY][WZ] grid must be cleared.  A warp
         //      takes every 4th word of the bitmap; a quarter-warp clears one slot with 8 conflict-free 16-byte stores ----
 #pragma unroll 1
@@ -365,7 +349,6 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         }
         if (gtid == 0) *reinterpret_cast<uint2 *>(sg + S::HDR_OFF) = make_uint2(hdr.x, hdr.y);
         __syncwarp();
-        SW_STAMP(gtid == 0, t, 2);
         // one arrival per warp; the group's first thread also announces the bytes of all the group's copies (the
         // count may run negative until then: the phase cannot complete before this arrival)
         if (lane == 0) {
@@ -374,7 +357,6 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
             else
                 mbar_arrive(bar);
         }
-        SW_STAMP(gtid == 0, t, 3);
         stage += G;
         if (stage >= SW_STAGES) {   // G <= SW_STAGES: at most one wrap
             stage -= SW_STAGES;
@@ -387,10 +369,8 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         }
         if (t + G < nsteps) {   // this group's next step: its record was requested SW_LOOKAHEAD steps before it
             mbar_wait(rbar0 + 8u * rs, rparity);
-            SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 6);
             fetch_v(rs);
         }
-        SW_STAMP(gtid == 0 && (SW_EXP & 8), t, 7);
     }
 }
 
@@ -453,12 +433,10 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             const int t = t0 + PH;
             if (t >= nsteps) break;
             tm_wait_st();
-            SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 4);
             mbar_wait(full0 + 8u * stage, parity);
-            SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 5);
             const unsigned char *sp = smem + (size_t)stage * S::STAGE_BYTES;
             const uint2 hdr = *reinterpret_cast<const uint2 *>(sp + S::HDR_OFF);   // {modes | flags, column offset}
-            const int mode = (SW_EXP & 64) ? MODE_EMPTY : (int)((hdr.x >> (2 * warp)) & 3u);   // development, bit 6: consumers only wait and release
+            const int mode = (int)((hdr.x >> (2 * warp)) & 3u);
             const double *pb = reinterpret_cast<const double *>(sp + b0);
 
             // store offsets of the outputs this step completes (plane t - N), staged by the producer; -1: none
@@ -474,14 +452,11 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
 #pragma unroll
                 for (int j = 0; j < PY; ++j) {
                     uint32_t pw[N * 8];   // centre values of planes t-1 .. t-N of this patch row
-                    if (!(SW_EXP & 2)) tm_ld_row<N>(t_in + j * S::ROW_WORDS, pw);
-                    else
-#pragma unroll
-                        for (int q = 0; q < N * 8; ++q) pw[q] = io[q & 7] + q;
+                    tm_ld_row<N>(t_in + j * S::ROW_WORDS, pw);
                     double v[PZ + 2 * N];
 #pragma unroll
                     for (int tt = 0; tt < PZ + 2 * N; ++tt)
-                        v[tt] = (SW_EXP & 4) ? (tt == N ? pb[(j * WZ + tt) * SW_C] : (double)(tt + j) * w.w[1]) : pb[(j * WZ + tt) * SW_C];
+                        v[tt] = pb[(j * WZ + tt) * SW_C];
                     const double2 va = *reinterpret_cast<const double2 *>(sp + vrow + j * 128);
                     const double2 vb = *reinterpret_cast<const double2 *>(sp + vrow + j * 128 + 16);
                     const double vv[4] = {va.x, va.y, vb.x, vb.y};
@@ -493,7 +468,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
 #pragma unroll
                         for (int k = 1; k < N; ++k) acc[(PH + N - k) % N][j][i] = fma(w.w[k], ce, acc[(PH + N - k) % N][j][i]);
                         const double out = fma(w.w[N], ce, acc[PH][j][i]);
-                        if (!(SW_EXP & 1)) store_if_valid(hp, io[4 * j + i], out);
+                        store_if_valid(hp, io[4 * j + i], out);
                         s[i] = vv[i] * ce;   // vv = 3 w_0 + V, formed by the producer
 #pragma unroll
                         for (int k = 1; k <= N; ++k) {
@@ -502,7 +477,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                         }
                     }
                     // backward half of the x arm from tensor memory, then park this row's centre values
-                    if (!(SW_EXP & 2)) tm_wait_row<N>(pw);
+                    tm_wait_row<N>(pw);
 #pragma unroll
                     for (int i = 0; i < PZ; ++i) {
 #pragma unroll
@@ -518,7 +493,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                         cw[2 * i] = (uint32_t)__double2loint(ctr[j][i]);
                         cw[2 * i + 1] = (uint32_t)__double2hiint(ctr[j][i]);
                     }
-                    if (!(SW_EXP & 2)) tm_st8(t_in + j * S::ROW_WORDS + PH * 8, cw);
+                    tm_st8(t_in + j * S::ROW_WORDS + PH * 8, cw);
                 }
                 // y arms: rows ty0-N .. ty0+PY-1+N of the patch's 4 z columns
 #pragma unroll
@@ -526,8 +501,7 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
                     double u[PY + 2 * N];
 #pragma unroll
                     for (int tt = 0; tt < PY + 2 * N; ++tt)
-                        u[tt] = (tt >= N && tt < N + PY) ? ctr[tt - N][i]
-                                                         : ((SW_EXP & 4) ? (double)(tt + i) * w.w[1] : pb[((tt - N) * WZ + N + i) * SW_C]);
+                        u[tt] = (tt >= N && tt < N + PY) ? ctr[tt - N][i] : pb[((tt - N) * WZ + N + i) * SW_C];
 #pragma unroll
                     for (int j = 0; j < PY; ++j)
 #pragma unroll
@@ -571,7 +545,6 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             }
             // this warp has read everything it needs from the stage
             __syncwarp();
-            SW_STAMP(tid == 0 && !(SW_EXP & 8), t, 6);
             if (lane == 0) mbar_arrive(empty0 + 8u * stage);
             if (tid == 0 && step_clock) step_clock[t] = clock64();
             if (++stage == SW_STAGES) {
@@ -654,35 +627,10 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
 // ---------------------------------------------------------------------------------------------
 // host: work pieces, their assignment to CTAs, and the per-step records
 // ---------------------------------------------------------------------------------------------
-static int g_max_planes = 32;   // x-slab thickness of a work item (rs_set_tuning("sweep_planes", v))
-static int g_tuned_planes = 1 << 20;   // the same once the step costs are measured (rs_set_tuning("sweep_planes_tuned", v)):
-                                       // with true costs the dealing balances whole tile columns, and fewer pieces mean
-                                       // fewer halo steps (measured on B200, config 2: 32 -> 0.148 ms, whole extent -> 0.140 ms)
-static int g_force_tensor = 0;  // rs_set_tuning("sweep_tensor", 1): use the tensor-map copies also for 16 columns (tests)
-static int g_nctas = 0;         // rs_set_tuning("sweep_ctas", v): persistent CTAs (0 = one per SM)
-static int g_min_split = 3;     // rs_set_tuning("sweep_min_split", v): fewest output planes of a piece cut off by the dealing
-static int g_tune_rounds = 3;   // rs_set_tuning("sweep_tune_rounds", v): measure / re-deal rounds of rs_hamiltonian_autotune
-static int g_shape = 0;         // rs_set_tuning("sweep_shape", 1): fd_order 4 on the 12-warp shape (experiment)
-void rs_sweep_set_max_planes(int v) { g_max_planes = v < 4 ? 4 : v; }
-void rs_sweep_set_tuned_planes(int v) { g_tuned_planes = v < 4 ? 4 : v; }
-void rs_sweep_set_force_tensor(int v) { g_force_tensor = v != 0; }
-void rs_sweep_set_nctas(int v) { g_nctas = v < 0 ? 0 : v; }
-void rs_sweep_set_shape(int v) { g_shape = v; }
-void rs_sweep_set_min_split(int v) { g_min_split = v < 1 ? 1 : v; }
-void rs_sweep_set_tune_rounds(int v) { g_tune_rounds = v < 1 ? 1 : v; }
-
 namespace {
-enum { VARIANT_N4 = 0, VARIANT_N6 = 1, VARIANT_N4W12 = 2, VARIANT_NONE = -1 };
-int sweep_variant(int n)
-{
-    if (n == 4) return g_shape == 1 ? VARIANT_N4W12 : VARIANT_N4;
-    if (n == 6) return VARIANT_N6;
-    return VARIANT_NONE;
-}
-shape_rt variant_shape(int variant)
-{
-    return variant == VARIANT_N6 ? shape_of<shape_n6>() : variant == VARIANT_N4W12 ? shape_of<shape_n4w12>() : shape_of<shape_n4>();
-}
+enum { VARIANT_N4 = 0, VARIANT_N6 = 1, VARIANT_NONE = -1 };
+int sweep_variant(int n) { return n == 4 ? VARIANT_N4 : n == 6 ? VARIANT_N6 : VARIANT_NONE; }
+shape_rt variant_shape(int variant) { return variant == VARIANT_N6 ? shape_of<shape_n6>() : shape_of<shape_n4>(); }
 }  // namespace
 
 namespace {
@@ -739,9 +687,9 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
     const shape_rt sh = variant_shape(variant);
     const int N = sh.N, TY = sh.TY, TZ = SW_TZ, WY = sh.WY, WZ = sh.WZ;
     tile_geometry g{m, sh, m->dims[0], m->dims[1], m->dims[2], (m->dims[1] + TY - 1) / TY, (m->dims[2] + TZ - 1) / TZ};
-    out.rec_bytes = sh.rec_bytes;
     const int nx = g.nx, nchunks = ncol / SW_C;
     out = rs_sweep_host();
+    out.rec_bytes = sh.rec_bytes;
 
     // ---- cost of every (tile, plane) as a full step; 0 where the tile has no mesh point in the plane ----
     std::vector<double> fcost((size_t)g.nty * g.ntz * nx, 0.0), ccost((size_t)g.nty * g.ntz * nx, 0.0);
@@ -812,7 +760,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
         pieces.assign(nctas, {});
         load.assign(nctas, 0.0);
         std::vector<char> closed(nctas, 0);   // CTAs that cannot take another piece without overshooting
-                const int MIN_SPLIT = g_min_split;    // output planes: below this the 2 N halo steps dominate
+        const int MIN_SPLIT = m->opt.min_split < 1 ? 1 : m->opt.min_split;   // output planes: below this the 2 N halo steps dominate
         auto least_loaded = [&](bool open_only) {
             int best = -1;
             for (int c = 0; c < nctas; ++c)
@@ -951,7 +899,8 @@ bool rs_sweep_supported(const rs_mesh *m, int n, int ncol)
            (uint64_t)(m->np + 1) * (uint64_t)ncol < 0xffffffffull;   // store offsets are 32-bit element offsets
 }
 
-static int sweep_nctas(const rs_mesh *m) { return g_nctas > 0 ? g_nctas : (m->sm_count > 0 ? m->sm_count : 148); }
+static int sweep_nctas(const rs_mesh *m) { return m->opt.ctas > 0 ? m->opt.ctas : (m->sm_count > 0 ? m->sm_count : 148); }
+static int clamp_planes(int v) { return v < 4 ? 4 : v; }
 
 template <class S>
 static cudaError_t set_smem()
@@ -979,7 +928,7 @@ static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables *
         rs_sweep_tables tb;
         const auto mc = m->sweep_costs.find(key);
         const bool tuned = mc != m->sweep_costs.end();
-        tb.ok = rs_sweep_build_host(m, n, ncol, tuned ? g_tuned_planes : g_max_planes, sweep_nctas(m), h, tuned ? &mc->second : nullptr);
+        tb.ok = rs_sweep_build_host(m, n, ncol, clamp_planes(tuned ? m->opt.planes_tuned : m->opt.planes), sweep_nctas(m), h, tuned ? &mc->second : nullptr);
         if (tb.ok) {
             tb.nitems = (int64_t)h.items.size();
             tb.nrec = h.nrec;
@@ -1001,13 +950,12 @@ static rs_status get_tables(rs_mesh *m, int n, int ncol, const rs_sweep_tables *
                 int64_t nfull = 0;
                 for (int t = 0; t < h.items[c].y; ++t) {
                     const uint32_t hd = *reinterpret_cast<const uint32_t *>(h.recs.data() + (size_t)(h.items[c].x + t) * h.rec_bytes + SW_REC_HDR);
-                    for (int wq = 0; wq < 12; ++wq) nfull += ((hd >> (2 * wq)) & 3u) == MODE_FULL;
+                    for (int wq = 0; wq < 8; ++wq) nfull += ((hd >> (2 * wq)) & 3u) == MODE_FULL;
                 }
                 tb.host_stats.insert(tb.host_stats.end(), {(int64_t)h.items[c].y, (int64_t)h.pieces[c].size(), (int64_t)(h.load[c] * 1000), nfull});
             }
             RS_CUDA_TRY(set_smem<shape_n4>());
             RS_CUDA_TRY(set_smem<shape_n6>());
-            RS_CUDA_TRY(set_smem<shape_n4w12>());
         }
         f = m->sweep.emplace(key, tb).first;
     }
@@ -1043,10 +991,33 @@ static rs_status encode_maps(const rs_mesh *m, const double *psi, int ncol, swee
     return RS_OK;
 }
 
-rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const double *vloc, const double *psi,
-                          double *hpsi, int ncol, cudaStream_t st)
+// The six tensor maps of a psi buffer are encoded once per (pointer, row pitch) and kept in the handle (a caller's
+// block loop alternates between a few buffers): a warm apply does no driver call besides the launch.
+static rs_status cached_maps(rs_mesh *m, const double *psi, int ncol, const sweep_maps **out)
 {
-    rs_mesh *m = const_cast<rs_mesh *>(cm);  // lazily filled cache inside the handle
+    for (rs_sweep_map_cache &e : m->map_cache)
+        if (e.psi == psi && e.ncol == ncol) {
+            *out = reinterpret_cast<const sweep_maps *>(e.bytes);
+            return RS_OK;
+        }
+    static_assert(sizeof(sweep_maps) <= sizeof(rs_sweep_map_cache::bytes), "tensor-map cache entry");
+    if (m->map_cache.size() >= 16) m->map_cache.erase(m->map_cache.begin());   // oldest first
+    m->map_cache.emplace_back();
+    rs_sweep_map_cache &e = m->map_cache.back();
+    e.psi = psi, e.ncol = ncol;
+    const rs_status rc = encode_maps(m, psi, ncol, *reinterpret_cast<sweep_maps *>(e.bytes));
+    if (rc != RS_OK) {
+        m->map_cache.pop_back();
+        return rc;
+    }
+    *out = reinterpret_cast<const sweep_maps *>(e.bytes);
+    return RS_OK;
+}
+
+// measure = true (rs_hamiltonian_autotune only): every CTA also records its clock at the end of every step.
+static rs_status launch_sweep(rs_mesh *m, int n, const rs_weights &w, const double *vloc, const double *psi, double *hpsi,
+                              int ncol, cudaStream_t st, bool measure)
+{
     if (!rs_sweep_supported(m, n, ncol)) return rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep kernel cannot serve this call");
     const rs_sweep_tables *tb = nullptr;
     rs_status rc = get_tables(m, n, ncol, &tb);
@@ -1055,26 +1026,40 @@ rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const d
     sweep_args a;
     a.items = tb->d_items, a.recs = tb->d_recs;
     a.vloc = vloc, a.psi = psi, a.hpsi = hpsi, a.ncol = (uint32_t)ncol;
-    a.cycles = tb->d_cycles;
-    a.step_clock = tb->d_step_clock;
-    sweep_maps maps;
-    const bool tensor = ncol != SW_C || g_force_tensor;
+    a.cycles = measure ? tb->d_cycles : nullptr;
+    a.step_clock = measure ? tb->d_step_clock : nullptr;
+    static const sweep_maps no_maps = {};
+    const sweep_maps *maps = &no_maps;
+    const bool tensor = ncol != SW_C || m->opt.force_tensor;
     if (tensor) {
-        if (((uintptr_t)psi & 15u) != 0) return rs_fail(RS_ERR_INVALID_ARG, "psi must be 16-byte aligned");
-        rc = encode_maps(m, psi, ncol, maps);
+        rc = cached_maps(m, psi, ncol, &maps);
         if (rc != RS_OK) return rc;
-    } else {
-        std::memset(&maps, 0, sizeof(maps));
     }
     const unsigned grid = (unsigned)tb->nitems;
     if (tb->variant == VARIANT_N6)
-        launch_shape<shape_n6>(tensor, grid, st, a, w, maps);
-    else if (tb->variant == VARIANT_N4W12)
-        launch_shape<shape_n4w12>(tensor, grid, st, a, w, maps);
+        launch_shape<shape_n6>(tensor, grid, st, a, w, *maps);
     else
-        launch_shape<shape_n4>(tensor, grid, st, a, w, maps);
+        launch_shape<shape_n4>(tensor, grid, st, a, w, *maps);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
+}
+
+rs_status rs_launch_sweep(const rs_mesh *cm, int n, const rs_weights &w, const double *vloc, const double *psi,
+                          double *hpsi, int ncol, cudaStream_t st)
+{
+    return launch_sweep(const_cast<rs_mesh *>(cm), n, w, vloc, psi, hpsi, ncol, st, false);   // the handle owns lazily filled caches
+}
+
+// Build and upload the tables of (mesh, n, ncol) now (rs_hamiltonian_prepare): afterwards rs_launch_sweep allocates
+// nothing and never synchronises.
+rs_status rs_sweep_prepare(const rs_mesh *cm, int n, int ncol)
+{
+    rs_mesh *m = const_cast<rs_mesh *>(cm);
+    if (!rs_sweep_supported(m, n, ncol)) return rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep kernel cannot serve this call");
+    const rs_sweep_tables *tb = nullptr;
+    rs_status rc = get_tables(m, n, ncol, &tb);
+    if (rc != RS_OK) return rc;
+    return tb->ok ? RS_OK : rs_fail(RS_ERR_UNSUPPORTED, "plane-sweep tables: a plane needs more copy runs than a record holds");
 }
 
 // true when the sweep kernel will really serve (mesh, n, ncol): supported and its tables could be built
@@ -1093,16 +1078,15 @@ int64_t rs_sweep_table_bytes(const rs_mesh *cm, int n, int ncol)
     auto f = m->sweep.find(std::make_pair(n * 16 + sweep_variant(n), ncol));
     if (f != m->sweep.end()) return f->second.bytes;
     rs_sweep_host h;   // no device (or not built yet): count on the host
-    if (!rs_sweep_build_host(m, n, ncol, g_max_planes, sweep_nctas(m), h)) return 0;
+    if (!rs_sweep_build_host(m, n, ncol, clamp_planes(m->opt.planes), sweep_nctas(m), h)) return 0;
     return (int64_t)(h.items.size() * sizeof(int2) + h.recs.size());
 }
 
-const char *rs_sweep_variant_name(const rs_mesh *, int n, int ncol)
+const char *rs_sweep_variant_name(const rs_mesh *m, int n, int ncol)
 {
-    const bool tensor = ncol != SW_C || g_force_tensor;
+    const bool tensor = ncol != SW_C || m->opt.force_tensor;
     switch (sweep_variant(n)) {
         case VARIANT_N6: return tensor ? "sweep[n6 c16 8x16 q2p4 persistent ws tma2d+tmem s3]" : "sweep[n6 c16 8x16 q2p4 persistent ws tma1d+tmem s3]";
-        case VARIANT_N4W12: return tensor ? "sweep[n4 c16 12x16 q2p4 persistent ws tma2d+tmem s3]" : "sweep[n4 c16 12x16 q2p4 persistent ws tma1d+tmem s3]";
         default: return tensor ? "sweep[n4 c16 16x16 q4p4 persistent ws tma2d+tmem s3]" : "sweep[n4 c16 16x16 q4p4 persistent ws tma1d+tmem s3]";
     }
 }
@@ -1114,6 +1098,7 @@ void rs_sweep_free(rs_mesh *m)
         cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles), cudaFree(t.d_step_clock);
     }
     m->sweep.clear();
+    m->map_cache.clear();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1239,11 +1224,6 @@ int64_t rs_sweep_read_stats(const rs_mesh *cm, int n, int ncol, int64_t *out, in
     const int64_t nc = std::min<int64_t>(t.nitems, max_ctas);
     std::vector<long long> cyc(t.nitems + 2048);
     if (cudaMemcpy(cyc.data(), t.d_cycles, cyc.size() * sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess) return 0;
-#ifdef SW_TRACE
-    if (max_ctas >= t.nitems + 410) {   // development builds: the timeline follows the per-CTA rows
-        for (int64_t q = 0; q < 2048; ++q) out[5 * t.nitems + q] = cyc[t.nitems + q];
-    }
-#endif
     for (int64_t c = 0; c < nc; ++c) {
         out[5 * c] = cyc[c];
         for (int k = 0; k < 4; ++k) out[5 * c + 1 + k] = t.host_stats[4 * c + k];
@@ -1264,13 +1244,13 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
     if (!rs_sweep_supported(m, n, ncol)) return RS_OK;   // the gather kernel serves this call: nothing to tune
     const auto key = std::make_pair(n * 16 + sweep_variant(n), ncol);
     rs_sweep_costs costs;
-    for (int round = 0; round < g_tune_rounds; ++round) {   // later rounds measure the re-dealt work and refine it
+    for (int round = 0; round < (m->opt.tune_rounds < 1 ? 1 : m->opt.tune_rounds); ++round) {   // later rounds measure the re-dealt work and refine it
         const rs_sweep_tables *tb = nullptr;
         rs_status rc = get_tables(m, n, ncol, &tb);
         if (rc != RS_OK) return rc;
         if (!tb->ok) return RS_OK;
         for (int rep = 0; rep < 3; ++rep) {
-            rc = rs_launch_sweep(m, n, w, vloc, psi, hpsi, ncol, st);
+            rc = launch_sweep(m, n, w, vloc, psi, hpsi, ncol, st, true);
             if (rc != RS_OK) return rc;
         }
         RS_CUDA_TRY(cudaStreamSynchronize(st));
@@ -1311,6 +1291,9 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
             m->sweep.erase(f);
         }
     }
-    const rs_sweep_tables *tb = nullptr;
-    return get_tables(m, n, ncol, &tb);
+    // one measuring launch on the final tables: rs_sweep_stats then describes the dealing now in use
+    rs_status rc = launch_sweep(m, n, w, vloc, psi, hpsi, ncol, st, true);
+    if (rc != RS_OK) return rc;
+    RS_CUDA_TRY(cudaStreamSynchronize(st));
+    return RS_OK;
 }

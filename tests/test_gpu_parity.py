@@ -79,20 +79,17 @@ def test_other_orders(n, kernel):
     check(g, o, p.cond_denominator(psi, n), f"order {n}")
 
 
-@pytest.mark.parametrize("knob", [("sweep_tensor", 1), ("sweep_planes", 8), ("sweep_planes", 100), ("sweep_ctas", 7),
-                                  ("sweep_ctas", 1000)])
+@pytest.mark.parametrize("knob", [("force_tensor", 1), ("planes", 8), ("planes", 100), ("ctas", 7), ("ctas", 1000)])
 def test_sweep_kernel_variants(knob):
-    """The plane-sweep kernel under its tuning knobs: 2-D tensor-map copies for 16 columns, thin and thick slabs,
+    """The plane-sweep kernel under its per-mesh options: 2-D tensor-map copies for 16 columns, thin and thick slabs,
     few CTAs (long chains of work pieces through one CTA) and more CTAs than work."""
     cfg = synthetic.config(1)
-    rs.rs_set_tuning(*knob)
-    try:
-        p = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=4)      # fresh mesh: tables built under the knob
-        psi = synthetic.orbitals(cfg.seed, 0, cfg.nst, p.np)
-        g = p.gpu_hpsi(psi, 4, 16, kernel=rs.RS_KERNEL_SWEEP)
-        assert rs.rs_kernel_name(p.mesh, 4, 16, kernel=rs.RS_KERNEL_SWEEP).startswith("sweep[")
-    finally:
-        rs.rs_set_tuning(knob[0], {"sweep_tensor": 0, "sweep_planes": 32, "sweep_ctas": 0}[knob[0]])
+    p = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=4)      # fresh mesh: its own options
+    rs.rs_mesh_set_sweep_options(p.mesh, **{knob[0]: knob[1]})
+    psi = synthetic.orbitals(cfg.seed, 0, cfg.nst, p.np)
+    g = p.gpu_hpsi(psi, 4, 16, kernel=rs.RS_KERNEL_SWEEP)
+    assert rs.rs_kernel_name(p.mesh, 4, 16, kernel=rs.RS_KERNEL_SWEEP).startswith("sweep[")
+    assert rs.rs_kernel_name(problem(1).mesh, 4, 16, kernel=rs.RS_KERNEL_SWEEP).count("tma2d") == 0   # other meshes keep the defaults
     o = problem(1).oracle_hpsi(psi, 4)
     check(g, o, problem(1).cond_denominator(psi, 4), f"sweep variant {knob}")
 
@@ -110,22 +107,6 @@ def test_sweep_kernel_order6(B, is_complex):
     assert rs.rs_kernel_name(p.mesh, 6, B, rs.RS_COMPLEX128 if is_complex else rs.RS_REAL64, rs.RS_KERNEL_SWEEP).startswith("sweep[n6")
     o = p.oracle_hpsi(psi, 6)
     check(g, o, p.cond_denominator(psi, 6), f"sweep n=6 B={B}")
-
-
-@pytest.mark.parametrize("B", [16, 32])
-def test_sweep_kernel_12_warp_shape(B):
-    """fd_order 4 on the experimental 12 x 16 / 2 x 4 shape with 12 consumer warps."""
-    cfg = synthetic.config(1)
-    rs.rs_set_tuning("sweep_shape", 1)
-    try:
-        p = Problem(cfg.centers, cfg.charges, cfg.radius, cfg.spacing, max_n=4)
-        psi = synthetic.orbitals(cfg.seed, 0, B + 1, p.np)
-        g = p.gpu_hpsi(psi, 4, B, kernel=rs.RS_KERNEL_SWEEP)
-        assert rs.rs_kernel_name(p.mesh, 4, B, kernel=rs.RS_KERNEL_SWEEP).startswith("sweep[n4 c16 12x16")
-    finally:
-        rs.rs_set_tuning("sweep_shape", 0)
-    o = problem(1).oracle_hpsi(psi, 4)
-    check(g, o, problem(1).cond_denominator(psi, 4), f"12-warp shape B={B}")
 
 
 def test_autotune_keeps_parity():
@@ -151,6 +132,8 @@ def test_autotune_keeps_parity():
     check(g, o, problem(1).cond_denominator(psi, 4), "after autotune")
     st = rs.rs_sweep_stats(p.mesh, 4, B)
     assert st.shape[0] > 0 and st[:, 0].max() > 0
+    # per-CTA regressors of the cost model (the "full warp-steps" column read record 0 for every step)
+    assert st[:, 4].sum() > 0 and (st[:, 4] <= 8 * st[:, 1]).all() and len(set(st[:, 4].tolist())) > 1
 
 
 @pytest.mark.parametrize("seed,n,B", [(0, 4, 16), (1, 4, 32), (2, 6, 16), (3, 6, 32)])
@@ -170,11 +153,8 @@ def test_sweep_kernel_ragged_clusters(seed, n, B):
     blk = torch.zeros((p.np + 1, B), dtype=torch.float64, device="cuda")
     hblk = torch.empty_like(blk)
     v = torch.from_numpy(p.v_mesh).cuda()
-    rs.rs_set_tuning("sweep_planes_tuned", 7)            # short pieces after the re-deal as well
-    try:
-        rs.rs_hamiltonian_autotune(p.mesh, n, oracle.fd_coeffs(n), v, blk, hblk, B)
-    finally:
-        rs.rs_set_tuning("sweep_planes_tuned", 1 << 20)
+    rs.rs_mesh_set_sweep_options(p.mesh, planes_tuned=7)   # short pieces after the re-deal as well
+    rs.rs_hamiltonian_autotune(p.mesh, n, oracle.fd_coeffs(n), v, blk, hblk, B)
     check(_run(p, psi, n, B, "sweep"), o, den, f"ragged seed {seed} n={n} B={B} after autotune")
 
 
@@ -314,6 +294,73 @@ def test_states_host_entry_point():
     check(p.to_canon(out), o, p.cond_denominator(psi, 4), "states_host")
 
 
+@pytest.mark.parametrize("B,nst,is_complex,ld_pad", [(4, 22, False, 3), (16, 70, False, 5), (64, 265, False, 0),
+                                                     (16, 70, True, 1), (4, 22, True, 0)])
+def test_states_stream_many_blocks(B, nst, is_complex, ld_pad):
+    """a7 on config 1 with >= 5 blocks and a ragged last one: every window of the 3-deep ring is reused (block 3
+    re-enters window 0), uploads / computes / downloads overlap on three streams, sweep kernel for B >= 16 real columns;
+    padded leading dimension: the caller's padding columns must come back untouched.  Second call on the same
+    workspace (nothing allocated) with other inputs."""
+    p = problem(1)
+    dt = rs.RS_COMPLEX128 if is_complex else rs.RS_REAL64
+    ld = p.np + ld_pad
+    ws = rs.rs_workspace_create(p.mesh, B, dt, ld)
+    assert ws.nbytes == 3 * 2 * (B * ld * (16 if is_complex else 8) + rs.rs_block_bytes(p.mesh, B, dt)) + 8 * p.np
+    for seed in (71, 72):
+        psi = synthetic.orbitals(seed, 0, nst, p.np, is_complex=is_complex)
+        st = np.full((nst, ld), 123.0, dtype=psi.dtype)
+        st[:, :p.np] = p.to_mesh(psi)
+        out = np.full((nst, ld), -7.0, dtype=psi.dtype)
+        rs.rs_hamiltonian_apply_states_stream(ws, 4, oracle.fd_coeffs(4), p.v_mesh, st, out)
+        assert np.all(out[:, p.np:] == -7.0)
+        o = p.oracle_hpsi(psi, 4, nthreads=16)
+        check(p.to_canon(out[:, :p.np]), o, p.cond_denominator(psi, 4), f"states_stream B={B} nst={nst} seed={seed}")
+    if B == 16 and not is_complex:                        # the convenience form (workspace per call) gives the same bits
+        out2 = np.full((nst, ld), -7.0, dtype=psi.dtype)
+        rs.rs_hamiltonian_apply_states_host(p.mesh, 4, oracle.fd_coeffs(4), p.v_mesh, st, out2, B)
+        assert np.array_equal(out, out2)
+
+
+def test_warm_apply_allocates_nothing():
+    """after rs_hamiltonian_prepare, apply / pack / unpack allocate nothing (free device memory
+    unchanged across many calls, also for a new psi buffer of a wide block whose tensor maps are host-side only)."""
+    import torch
+
+    p = problem(1)
+    dev = torch.device("cuda:0")
+    v = torch.from_numpy(p.v_mesh).to(dev)
+    c = oracle.fd_coeffs(4)
+    for B in (8, 16, 32):
+        bufs = [torch.zeros((p.np + 1, B), dtype=torch.float64, device=dev) for _ in range(4)]
+        rs.rs_hamiltonian_prepare(p.mesh, 4, B)
+        torch.cuda.synchronize()
+        free0 = torch.cuda.mem_get_info()[0]
+        for k in range(6):
+            rs.rs_hamiltonian_apply(p.mesh, 4, c, v, bufs[k % 2], bufs[2 + k % 2], B)
+        torch.cuda.synchronize()
+        assert torch.cuda.mem_get_info()[0] == free0, f"apply allocated device memory (B={B})"
+
+
+def test_misaligned_block_pointers_are_rejected():
+    """psi / hpsi must be 16-byte aligned on every kernel path: an offset view returns RS_ERR_INVALID_ARG
+    instead of faulting in a bulk copy."""
+    import torch
+
+    p = problem(1)
+    dev = torch.device("cuda:0")
+    v = torch.from_numpy(p.v_mesh).to(dev)
+    for B in (1, 16, 32):
+        raw = torch.zeros((p.np + 1) * B + 2, dtype=torch.float64, device=dev)
+        ok = torch.zeros((p.np + 1) * B, dtype=torch.float64, device=dev)
+        off = raw[1:1 + (p.np + 1) * B]
+        assert off.data_ptr() % 16 == 8
+        for psi, hpsi in ((off, ok), (ok, off)):
+            with pytest.raises(rs.RsError) as e:
+                rs.rs_hamiltonian_apply(p.mesh, 4, oracle.fd_coeffs(4), v, psi, hpsi, B)
+            assert e.value.status == rs.RS_ERR_INVALID_ARG
+    torch.cuda.synchronize()                              # no sticky fault
+
+
 def test_kernel_choice_is_reported():
     p = problem(1)
     name = rs.rs_kernel_name(p.mesh, 4, 16)
@@ -324,35 +371,61 @@ def test_kernel_choice_is_reported():
 # ---- full-size configs (BASELINE.json configs[2..4]) in the launch configuration bench.py times -----------
 # One block of orbitals through pack -> apply -> unpack on the full mesh, every output compared with the
 # oracle (the oracle does a whole orbital of these meshes in a fraction of a second per core).
-@pytest.mark.parametrize("B", [16, 32, 64])
+@pytest.mark.parametrize("B", [1, 2, 4, 8, 16, 32, 64])
 def test_config2_full_mesh_block(B):
+    """Every block size BASELINE.json configs[2] names, on the full 1.96 M-point mesh (B < 16: the gather kernel)."""
     p = problem(2)
     cfg = p.cfg
     nst = B + 3 if B == 16 else B                       # B = 16: a second, ragged block as well
     psi = synthetic.orbitals(cfg.seed, 0, nst, p.np)
     g = _run(p, psi, 4, B, "auto")
-    assert rs.rs_kernel_name(p.mesh, 4, B).startswith("sweep[")
+    assert rs.rs_kernel_name(p.mesh, 4, B).startswith("sweep[" if B >= 16 else "gather")
     o = p.oracle_hpsi(psi, 4, nthreads=16)
     check(g, o, p.cond_denominator(psi, 4), f"config2 B={B}")
 
 
-@pytest.mark.parametrize("B", [8, 32])
+@pytest.mark.parametrize("B", [1, 2, 4, 8, 16, 32])
 def test_config3_complex_full_mesh_block(B):
+    """Every block size BASELINE.json configs[3] names (complex: 2 B real columns; B < 8: the gather kernel)."""
     p = problem(2)                                       # config 3 = config 2's mesh and potential, complex orbitals
     cfg = synthetic.config(3)
     psi = synthetic.orbitals(cfg.seed, 0, B, p.np, is_complex=True)
     g = _run(p, psi, 4, B, "auto")
-    assert rs.rs_kernel_name(p.mesh, 4, B, rs.RS_COMPLEX128).startswith("sweep[")
+    assert rs.rs_kernel_name(p.mesh, 4, B, rs.RS_COMPLEX128).startswith("sweep[" if B >= 8 else "gather")
     o = p.oracle_hpsi(psi, 4, nthreads=16)
     check(g, o, p.cond_denominator(psi, 4), f"config3 complex B={B}")
 
 
-@pytest.mark.parametrize("n,B", [(4, 16), (4, 64), (6, 16)])
+@pytest.mark.parametrize("n,B", [(4, 16), (4, 32), (4, 64), (6, 16), (6, 32), (6, 64)])
 def test_config4_full_mesh_block(n, B):
-    p = problem(4)                                       # 500 centres, 3.8 M points; orders 4 and 6
+    """BASELINE.json configs[4]: blocks of 16 / 32 / 64 REAL orbitals (no padding columns), orders 4 and 6."""
+    p = problem(4)                                       # 500 centres, 3.8 M points
     cfg = p.cfg
-    nst = min(B, 16)                                     # 16 orbitals (padded block for B = 64): the oracle's share stays small
-    psi = synthetic.orbitals(cfg.seed, 0, nst, p.np)
+    psi = synthetic.orbitals(cfg.seed, 0, B, p.np)
     g = _run(p, psi, n, B, "auto")
+    assert rs.rs_kernel_name(p.mesh, n, B).startswith(f"sweep[n{n}")
     o = p.oracle_hpsi(psi, n, nthreads=16)
     check(g, o, p.cond_denominator(psi, n), f"config4 n={n} B={B}")
+
+
+def test_config4_streamed_at_its_stated_size():
+    """BASELINE.json configs[4] end to end: 1024 real orbitals streamed through HBM in blocks of 64, fd_order 4, through
+    the a7 workspace (3 windows: the device never holds more than 3 blocks).  Orbitals are generated chunk by chunk on
+    the host (neither side holds the 31 GB set); one sampled orbital per 128 is compared with the oracle."""
+    p = problem(4)
+    cfg = p.cfg
+    B, chunk, n = 64, 128, 4
+    ws = rs.rs_workspace_create(p.mesh, B, rs.RS_REAL64, p.np)
+    c = oracle.fd_coeffs(n)
+    rng = np.random.default_rng(4)
+    worst = 0.0
+    for ist0 in range(0, cfg.nst, chunk):
+        psi = synthetic.orbitals(cfg.seed, ist0, chunk, p.np)
+        st = p.to_mesh(psi)
+        out = np.empty_like(st)
+        rs.rs_hamiltonian_apply_states_stream(ws, n, c, p.v_mesh, st, out)
+        j = int(rng.integers(0, chunk))                  # a seeded sample: orbital ist0 + j
+        o = p.oracle_hpsi(psi[j:j + 1], n, nthreads=16)
+        worst = max(worst, check(p.to_canon(out[j:j + 1]), o, p.cond_denominator(psi[j:j + 1], n), f"config4 orbital {ist0 + j}"))
+        assert np.isfinite(out).all()
+    assert worst <= 1e-12

@@ -192,6 +192,25 @@ def test_no_cpu_fallback_without_a_device():
     assert e.value.status == rs.RS_ERR_CUDA
 
 
+def test_misaligned_block_pointers_are_rejected_without_a_device():
+    """Argument checks come before the device check: a psi / hpsi pointer that is not 16-byte aligned (an offset view)
+    is RS_ERR_INVALID_ARG on every kernel path (rs.h "Alignment")."""
+    m = rs.rs_mesh_create_box(8, 8, 8, 0.25, 4)
+    npts = m.npoints
+    c = np.array([-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560])
+    for B in (1, 16, 32):
+        raw = np.zeros((npts + 1) * B + 4)
+        base = 0 if raw.ctypes.data % 16 == 0 else 1
+        ok, off = raw[base:base + (npts + 1) * B], raw[base + 1:base + 1 + (npts + 1) * B]
+        other = np.zeros((npts + 1) * B + 2)
+        other = other[(0 if other.ctypes.data % 16 == 0 else 1):][:(npts + 1) * B]
+        assert off.ctypes.data % 16 == 8 and ok.ctypes.data % 16 == 0 and other.ctypes.data % 16 == 0
+        for psi, hpsi in ((off, other), (other, off)):
+            with pytest.raises(rs.RsError) as e:
+                rs.rs_hamiltonian_apply(m, 4, c, np.zeros(npts), psi, hpsi, B, rs.RS_REAL64, stream=0)
+            assert e.value.status == rs.RS_ERR_INVALID_ARG
+
+
 # ---- plane-sweep kernel's compact records: host replay against the plain neighbour table (reading S15) ----
 @pytest.mark.parametrize("cfg_i,nst,dtype,planes,nctas", [
     (0, 16, rs.RS_REAL64, 32, 148), (0, 16, rs.RS_REAL64, 8, 3), (1, 16, rs.RS_REAL64, 32, 148),
@@ -205,17 +224,29 @@ def test_sweep_records_expand_to_the_plain_table(cfg_i, nst, dtype, planes, ncta
     assert st["nctas"] == nctas and st["records"] > 0 and st["cost_max"] >= st["cost_mean"] > 0
 
 
-@pytest.mark.parametrize("cfg_i,n,nst,shape", [(0, 6, 16, 0), (1, 6, 16, 0), (1, 6, 64, 0), (1, 4, 16, 1), (1, 4, 32, 1)])
-def test_sweep_records_other_kernel_shapes(cfg_i, n, nst, shape):
-    """fd_order 6 (8 x 16 tiles, 2 x 4 patches) and the 12-warp shape for fd_order 4 (12 x 16 tiles)."""
+@pytest.mark.parametrize("cfg_i,n,nst", [(0, 6, 16), (1, 6, 16), (1, 6, 64)])
+def test_sweep_records_order6_shape(cfg_i, n, nst):
+    """fd_order 6 runs on its own kernel shape (8 x 16 tiles, 2 x 4 patches)."""
     cfg = synthetic.config(cfg_i)
     mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, 6)
-    rs.rs_set_tuning("sweep_shape", shape)
-    try:
-        st = rs.rs_sweep_selfcheck(mesh, n, nst, rs.RS_REAL64, 32, 148)
-    finally:
-        rs.rs_set_tuning("sweep_shape", 0)
+    st = rs.rs_sweep_selfcheck(mesh, n, nst, rs.RS_REAL64, 32, 148)
     assert st["records"] > 0
+
+
+def test_sweep_options_are_per_mesh():
+    """No process-global tuning state: options live in the mesh handle."""
+    d = rs.rs_sweep_options_default()
+    assert (d.planes, d.planes_tuned, d.ctas, d.force_tensor, d.min_split, d.tune_rounds) == (32, 1 << 20, 0, 0, 3, 3)
+    a = rs.rs_mesh_create_box(24, 24, 24, 0.25, 4)
+    b = rs.rs_mesh_create_box(24, 24, 24, 0.25, 4)
+    rs.rs_mesh_set_sweep_options(a, force_tensor=1, ctas=5)
+    assert "tma2d" in rs.rs_kernel_name(a, 4, 16, kernel=rs.RS_KERNEL_SWEEP)
+    assert "tma1d" in rs.rs_kernel_name(b, 4, 16, kernel=rs.RS_KERNEL_SWEEP)
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_mesh_set_sweep_options(a, planes=0)
+    assert e.value.status == rs.RS_ERR_INVALID_ARG
+    with pytest.raises(rs.RsError):
+        rs.rs_mesh_set_sweep_options(a, no_such_field=1)
 
 
 def test_sweep_selfcheck_on_boxes_and_unsupported_calls():
