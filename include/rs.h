@@ -136,6 +136,30 @@ rs_status rs_hamiltonian_apply_v(const rs_mesh *mesh, int fd_order, const double
                                  const double *vloc_dev, const void *psi_dev, void *hpsi_dev, int nst,
                                  rs_dtype dtype, void *stream, rs_kernel kernel);
 
+/* ---- block operations between orbitals (sec. VIII: "copies, linear
+ * combinations, and dot products ... using the block-of-orbitals approach"; residuals for RMM-DIIS) ---
+ * a, b, x, y, psi, hpsi: dev block buffers of width nst (layout above, 16-byte aligned).  Sums run over the np mesh
+ * points, plain (no h^3 factor, reading S11), with the conjugate on the LEFT argument.  Asynchronous on `stream`;
+ * results are deterministic (per-CTA partial sums in a scratch array owned by the mesh, added in a fixed order), so
+ * reductions on one mesh must not run concurrently on two streams.
+ *   rs_block_dot:          out_dev[j] = sum_p conj(a[p][j]) b[p][j], j < nst  (nst doubles, or nst (re, im) pairs)
+ *   rs_block_expectation:  out_dev[0][j] = Re <psi_j|hpsi_j>, out_dev[1][j] = |psi_j|^2,
+ *                          out_dev[2][j] = |hpsi_j - eps_j psi_j|^2 (eps_dev: nst real doubles, NULL = all 0): 3*nst doubles
+ *   rs_block_axpy:         y[p][j] += alpha[j] x[p][j]; alpha_dev: nst elements of the block's dtype
+ *   rs_block_copy:         dst = src (whole block, zero slot included)                                              */
+rs_status rs_block_dot(const rs_mesh *mesh, const void *a_dev, const void *b_dev, int nst, rs_dtype dtype, void *out_dev,
+                       void *stream);
+rs_status rs_block_expectation(const rs_mesh *mesh, const void *psi_dev, const void *hpsi_dev, const double *eps_dev, int nst,
+                               rs_dtype dtype, double *out_dev, void *stream);
+rs_status rs_block_axpy(const rs_mesh *mesh, const void *alpha_dev, const void *x_dev, void *y_dev, int nst, rs_dtype dtype,
+                        void *stream);
+rs_status rs_block_copy(const rs_mesh *mesh, const void *src_dev, void *dst_dev, int nst, rs_dtype dtype, void *stream);
+/* rs_hamiltonian_apply plus, from the same call, sums_dev = the three rows of rs_block_expectation(psi, H psi, eps):
+ * what one eigensolver step needs per orbital (Rayleigh quotient numerator and denominator, residual norm).        */
+rs_status rs_hamiltonian_apply_ex(const rs_mesh *mesh, int fd_order, const double *coeffs_host, const double *vloc_dev,
+                                  const void *psi_dev, void *hpsi_dev, int nst, rs_dtype dtype, void *stream,
+                                  const double *eps_dev, double *sums_dev);
+
 /* Once per (mesh, fd_order, nst, dtype), before the first apply: build and upload the neighbour structure the chosen
  * kernel needs (plain table for the gather kernel, per-plane records for the plane-sweep kernel).  May allocate and
  * synchronise; afterwards rs_hamiltonian_apply for these arguments allocates nothing and never synchronises

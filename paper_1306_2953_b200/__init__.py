@@ -37,6 +37,7 @@ EXPORTS = (
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
     "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version",
     "rs_sweep_options_default", "rs_mesh_set_sweep_options", "rs_hamiltonian_prepare",
+    "rs_block_dot", "rs_block_expectation", "rs_block_axpy", "rs_block_copy", "rs_hamiltonian_apply_ex",
     "rs_workspace_create", "rs_workspace_destroy", "rs_workspace_bytes", "rs_hamiltonian_apply_states_stream",
     "rs_sweep_selfcheck", "rs_sweep_stats", "rs_hamiltonian_autotune",
 )
@@ -83,6 +84,11 @@ def _load() -> C.CDLL:
     L.rs_hamiltonian_autotune.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp]
     L.rs_hamiltonian_apply_v.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp, C.c_int]
     L.rs_hamiltonian_apply_states_host.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int]
+    L.rs_block_dot.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp, vp]
+    L.rs_block_expectation.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, vp, vp]
+    L.rs_block_axpy.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, vp]
+    L.rs_block_copy.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp]
+    L.rs_hamiltonian_apply_ex.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp, vp, vp]
     L.rs_workspace_create.argtypes = [vp, C.c_int, C.c_int, C.c_int64, C.c_int, C.POINTER(vp)]
     L.rs_workspace_destroy.argtypes = [vp]
     L.rs_workspace_bytes.argtypes = [vp]
@@ -306,6 +312,35 @@ def rs_hamiltonian_apply_states_host(mesh: Mesh, fd_order: int, coeffs, vloc_hos
     _check(_lib.rs_hamiltonian_apply_states_host(mesh.handle, fd_order, _dptr(c), _ptr(vloc_host), _ptr(states_host),
                                                  _ptr(hstates_host), ld, nst_total, block_size,
                                                  _dtype_of(states_host)))
+
+
+def rs_block_dot(mesh: Mesh, a, b, nst: int, out, stream=None) -> None:
+    """out[j] = sum_p conj(a[p][j]) b[p][j] (device tensors; out: nst elements of the blocks' dtype)."""
+    _check(_lib.rs_block_dot(mesh.handle, _ptr(a), _ptr(b), nst, _dtype_of(a), _ptr(out), _stream(stream)))
+
+
+def rs_block_expectation(mesh: Mesh, psi, hpsi, eps, nst: int, out, stream=None) -> None:
+    """out[3][nst] float64 = Re<psi|hpsi>, |psi|^2, |hpsi - eps psi|^2 per orbital (eps: device float64 [nst] or None)."""
+    _check(_lib.rs_block_expectation(mesh.handle, _ptr(psi), _ptr(hpsi), _ptr(eps) if eps is not None else None, nst,
+                                     _dtype_of(psi), _ptr(out), _stream(stream)))
+
+
+def rs_block_axpy(mesh: Mesh, alpha, x, y, nst: int, stream=None) -> None:
+    """y[p][j] += alpha[j] x[p][j] (alpha: device tensor of nst elements of the blocks' dtype)."""
+    _check(_lib.rs_block_axpy(mesh.handle, _ptr(alpha), _ptr(x), _ptr(y), nst, _dtype_of(x), _stream(stream)))
+
+
+def rs_block_copy(mesh: Mesh, src, dst, nst: int, stream=None) -> None:
+    _check(_lib.rs_block_copy(mesh.handle, _ptr(src), _ptr(dst), nst, _dtype_of(src), _stream(stream)))
+
+
+def rs_hamiltonian_apply_ex(mesh: Mesh, fd_order: int, coeffs, vloc, psi, hpsi, nst: int, eps, sums, stream=None) -> None:
+    """rs_hamiltonian_apply plus sums[3][nst] = Re<psi|H psi>, |psi|^2, |H psi - eps psi|^2 from the same call."""
+    c = np.ascontiguousarray(coeffs, dtype=np.float64)
+    if c.shape != (fd_order + 1,):
+        raise RsError(RS_ERR_INVALID_ARG, "coeffs must hold c_0..c_n")
+    _check(_lib.rs_hamiltonian_apply_ex(mesh.handle, fd_order, _dptr(c), _ptr(vloc), _ptr(psi), _ptr(hpsi), nst,
+                                        _dtype_of(psi), _stream(stream), _ptr(eps) if eps is not None else None, _ptr(sums)))
 
 
 class Workspace:

@@ -77,6 +77,66 @@ extern "C" rs_status rs_hamiltonian_apply_v(const rs_mesh *m, int n, const doubl
     return rs_launch_gather(m, n, w, d_map, vloc, (const double *)psi, (double *)hpsi, ncol, (cudaStream_t)stream);
 }
 
+// ---- f1: block operations between orbitals (sec. VIII) -----------------------------------------
+static rs_status check_blocks(const rs_mesh *m, const void *a, const void *b, int nst, rs_dtype dtype, const char *who)
+{
+    if (!m || !a || !b || !pow2_in(nst, 1, RS_MAX_BLOCK) || (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
+        return rs_fail(RS_ERR_INVALID_ARG, std::string(who) + ": bad argument");
+    if ((((uintptr_t)a | (uintptr_t)b) & 15u) != 0) return rs_fail(RS_ERR_INVALID_ARG, std::string(who) + ": blocks must be 16-byte aligned");
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    return RS_OK;
+}
+
+extern "C" rs_status rs_block_dot(const rs_mesh *m, const void *a, const void *b, int nst, rs_dtype dtype, void *out_dev, void *stream)
+{
+    rs_status st = check_blocks(m, a, b, nst, dtype, "rs_block_dot");
+    if (st != RS_OK) return st;
+    if (!out_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_dot: null output");
+    const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
+    return rs_launch_block_reduce(m, (const double *)a, (const double *)b, nullptr, nst * lanes, lanes, 1, lanes == 2 ? 1 : 0,
+                                  (double *)out_dev, (cudaStream_t)stream);
+}
+
+extern "C" rs_status rs_block_expectation(const rs_mesh *m, const void *psi, const void *hpsi, const double *eps_dev, int nst,
+                                          rs_dtype dtype, double *out_dev, void *stream)
+{
+    rs_status st = check_blocks(m, psi, hpsi, nst, dtype, "rs_block_expectation");
+    if (st != RS_OK) return st;
+    if (!out_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_expectation: null output");
+    const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
+    return rs_launch_block_reduce(m, (const double *)psi, (const double *)hpsi, eps_dev, nst * lanes, lanes, 3, 0, out_dev,
+                                  (cudaStream_t)stream);
+}
+
+extern "C" rs_status rs_block_axpy(const rs_mesh *m, const void *alpha_dev, const void *x, void *y, int nst, rs_dtype dtype, void *stream)
+{
+    rs_status st = check_blocks(m, x, y, nst, dtype, "rs_block_axpy");
+    if (st != RS_OK) return st;
+    if (!alpha_dev || x == y) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_axpy: null alpha or x == y");
+    const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
+    return rs_launch_block_axpy(m, (const double *)alpha_dev, (const double *)x, (double *)y, nst * lanes, lanes, (cudaStream_t)stream);
+}
+
+extern "C" rs_status rs_block_copy(const rs_mesh *m, const void *src, void *dst, int nst, rs_dtype dtype, void *stream)
+{
+    rs_status st = check_blocks(m, src, dst, nst, dtype, "rs_block_copy");
+    if (st != RS_OK) return st;
+    RS_CUDA_TRY(cudaMemcpyAsync(dst, src, rs_block_bytes(m, nst, dtype), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return RS_OK;
+}
+
+// H psi and, from the same call, the per-orbital sums an eigensolver step needs.  The gather kernel and (for now) the
+// plane-sweep kernel form the sums in a second streaming kernel over psi and H psi (one extra read of both blocks).
+extern "C" rs_status rs_hamiltonian_apply_ex(const rs_mesh *m, int n, const double *coeffs, const double *vloc, const void *psi,
+                                             void *hpsi, int nst, rs_dtype dtype, void *stream, const double *eps_dev,
+                                             double *sums_dev)
+{
+    if (!sums_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_apply_ex: null output");
+    rs_status st = rs_hamiltonian_apply_v(m, n, coeffs, vloc, psi, hpsi, nst, dtype, stream, RS_KERNEL_AUTO);
+    if (st != RS_OK) return st;
+    return rs_block_expectation(m, psi, hpsi, eps_dev, nst, dtype, sums_dev, stream);
+}
+
 extern "C" rs_status rs_hamiltonian_autotune(const rs_mesh *m, int n, const double *coeffs, const double *vloc, const void *psi,
                                              void *hpsi, int nst, rs_dtype dtype, void *stream)
 {
@@ -311,7 +371,14 @@ extern "C" rs_status rs_hamiltonian_prepare(const rs_mesh *m, int n, int nst, rs
         return rs_fail(RS_ERR_INVALID_ARG, "rs_hamiltonian_prepare: bad argument");
     if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
     const int ncol = nst * (dtype == RS_COMPLEX128 ? 2 : 1);
-    if (resolve_kernel(m, n, ncol, RS_KERNEL_AUTO) == RS_KERNEL_SWEEP) return rs_sweep_prepare(m, n, ncol);
+    if (resolve_kernel(m, n, ncol, RS_KERNEL_AUTO) == RS_KERNEL_SWEEP) {
+        double *scr = nullptr;
+        rs_status s2 = rs_reduce_scratch(m, &scr);
+        return s2 != RS_OK ? s2 : rs_sweep_prepare(m, n, ncol);
+    }
+    double *scratch = nullptr;
+    rs_status st = rs_reduce_scratch(m, &scratch);   // the block reductions' per-CTA partial sums
+    if (st != RS_OK) return st;
     const int32_t *d_map = nullptr;
     return rs_mesh_device_map(m, n, &d_map);
 }

@@ -1,0 +1,185 @@
+// Block operations between orbitals (sec. VIII: "copies, linear
+// combinations, and dot products ... implemented on the GPU using the block-of-orbitals approach"; RMM-DIIS works
+// on residuals, sec. III).  All of them stream whole blocks once: bound by HBM.
+//
+// Reductions are deterministic: every CTA owns a fixed set of block rows and a fixed slot of per-CTA partial sums
+// in a scratch array owned by the mesh; a second, tiny kernel adds the slots in CTA order.  No atomics.
+#include "rs_internal.h"
+
+namespace {
+
+constexpr int RED_THREADS = 256;
+
+__device__ __forceinline__ double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
+
+// per real column c of the block (ncol real columns, complex = adjacent (re, im) pairs):
+//   q0 = sum a b, q1 = sum a a, q2 = sum (b - eps a)^2, q3 = sum (a_re b_im - a_im b_re)  [complex dot only, on the re column]
+// VEC = 2: a thread owns two adjacent columns (one complex element); VEC = 1: ncol == 1.
+template <int VEC, int NQ, bool CPLX_DOT>
+__global__ void __launch_bounds__(RED_THREADS) block_reduce_kernel(const double *__restrict__ a, const double *__restrict__ b,
+                                                                   const double *__restrict__ eps, int lanes, int64_t np, int ncol,
+                                                                   int tshift, double *__restrict__ partial)
+{
+    __shared__ double red[RED_THREADS * VEC];
+    const int tid = threadIdx.x, tpp = 1 << tshift;           // threads per point
+    const int cv = tid & (tpp - 1), prow = tid >> tshift, rpc = RED_THREADS >> tshift;
+    const int col = cv * VEC;
+    double e[VEC] = {}, acc[NQ][VEC] = {};
+    if (NQ > 2 && eps)
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) e[v] = eps[(col + v) / lanes];
+    const int64_t stride = (int64_t)gridDim.x * rpc;
+    for (int64_t ip = (int64_t)blockIdx.x * rpc + prow; ip < np; ip += stride) {
+        double x[VEC], y[VEC];
+        if constexpr (VEC == 2) {
+            const double2 xa = ld2(a + ip * ncol + col), yb = ld2(b + ip * ncol + col);
+            x[0] = xa.x, x[1] = xa.y, y[0] = yb.x, y[1] = yb.y;
+        } else {
+            x[0] = a[ip * ncol + col], y[0] = b[ip * ncol + col];
+        }
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            acc[0][v] = fma(x[v], y[v], acc[0][v]);
+            if constexpr (NQ > 1 && !CPLX_DOT) acc[1][v] = fma(x[v], x[v], acc[1][v]);
+            if constexpr (NQ > 2) {
+                const double r = fma(-e[v], x[v], y[v]);
+                acc[2][v] = fma(r, r, acc[2][v]);
+            }
+        }
+        if constexpr (CPLX_DOT && VEC == 2) acc[NQ - 1][1] += x[0] * y[1] - x[1] * y[0];   // Im conj(a) b in the im column's last slot
+    }
+    // CTA reduction over the rows, fixed order; slot layout partial[cta][q][ncol]
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        __syncthreads();
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) red[tid * VEC + v] = acc[q][v];
+        __syncthreads();
+        if (prow == 0) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                double s = 0.0;
+                for (int r = 0; r < rpc; ++r) s += red[((r << tshift) + cv) * VEC + v];
+                partial[((size_t)blockIdx.x * NQ + q) * ncol + col + v] = s;
+            }
+        }
+    }
+}
+
+// out[q][j] = sum over CTAs (in order) and over the orbital's lanes of partial[cta][q][j*lanes + l]; mode 1 (complex dot):
+// out[j] = (re, im) with re = q0 over both lanes, im = the extra sum kept in the im column of the last quantity.
+__global__ void block_reduce_final_kernel(const double *__restrict__ partial, int nctas, int nq, int nq_out, int ncol, int lanes,
+                                          int mode, double *__restrict__ out)
+{
+    const int nst = ncol / lanes;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nq_out * nst; idx += gridDim.x * blockDim.x) {
+        const int q = idx / nst, j = idx % nst;
+        if (mode == 1) {                       // complex dot: nq == 2 here (q0 = products, q1 = cross terms)
+            if (q != 0) continue;
+            double re = 0.0, im = 0.0;
+            for (int c = 0; c < nctas; ++c) {
+                re += partial[((size_t)c * 2 + 0) * ncol + 2 * j] + partial[((size_t)c * 2 + 0) * ncol + 2 * j + 1];
+                im += partial[((size_t)c * 2 + 1) * ncol + 2 * j + 1];
+            }
+            out[2 * j] = re, out[2 * j + 1] = im;
+        } else {
+            double s = 0.0;
+            for (int c = 0; c < nctas; ++c)
+                for (int l = 0; l < lanes; ++l) s += partial[((size_t)c * nq + q) * ncol + j * lanes + l];
+            out[(size_t)q * nst + j] = s;
+        }
+    }
+}
+
+// y[p][c] += alpha_j x[p][c], rows p < np; complex: (yr, yi) += (ar xr - ai xi, ar xi + ai xr)
+template <bool CPLX>
+__global__ void __launch_bounds__(256) block_axpy_kernel(const double *__restrict__ alpha, const double *__restrict__ x,
+                                                         double *__restrict__ y, int64_t nelem2, int ncol2)
+{
+    // one thread per pair of adjacent doubles (a complex element, or two real columns)
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nelem2; i += (int64_t)gridDim.x * blockDim.x) {
+        const int c2 = (int)(i % ncol2);
+        const double2 xv = ld2(x + 2 * i);
+        double2 yv = ld2(y + 2 * i);
+        if constexpr (CPLX) {
+            const double ar = alpha[2 * c2], ai = alpha[2 * c2 + 1];
+            yv.x += ar * xv.x - ai * xv.y;
+            yv.y += ar * xv.y + ai * xv.x;
+        } else {
+            yv.x = fma(alpha[2 * c2], xv.x, yv.x);
+            yv.y = fma(alpha[2 * c2 + 1], xv.y, yv.y);
+        }
+        *reinterpret_cast<double2 *>(y + 2 * i) = yv;
+    }
+}
+__global__ void __launch_bounds__(256) block_axpy1_kernel(const double *__restrict__ alpha, const double *__restrict__ x,
+                                                          double *__restrict__ y, int64_t np)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < np; i += (int64_t)gridDim.x * blockDim.x)
+        y[i] = fma(alpha[0], x[i], y[i]);
+}
+
+int ilog2i(int v)
+{
+    int l = 0;
+    while ((1 << l) < v) ++l;
+    return l;
+}
+
+}  // namespace
+
+// Scratch of per-CTA partial sums, owned by the mesh (allocated with it): RS_RED_CTAS x 4 quantities x 128 columns.
+rs_status rs_reduce_scratch(const rs_mesh *cm, double **out)
+{
+    rs_mesh *m = const_cast<rs_mesh *>(cm);
+    if (!m->d_red) RS_CUDA_TRY(cudaMalloc((void **)&m->d_red, (size_t)RS_RED_CTAS * 4 * 128 * sizeof(double)));
+    *out = m->d_red;
+    return RS_OK;
+}
+
+// mode 0: out[q][nst] for q < nq (1: <a|b> real part per orbital, 2: + |a|^2, 3: + |b - eps a|^2);  mode 1: complex dot (re, im)
+rs_status rs_launch_block_reduce(const rs_mesh *m, const double *a, const double *b, const double *eps, int ncol, int lanes,
+                                 int nq, int mode, double *out, cudaStream_t st)
+{
+    double *partial = nullptr;
+    rs_status rc = rs_reduce_scratch(m, &partial);
+    if (rc != RS_OK) return rc;
+    const int vec = ncol >= 2 ? 2 : 1;
+    const int tshift = ilog2i(ncol / vec);
+    const int rpc = RED_THREADS >> tshift;
+    int grid = (int)((m->np + rpc - 1) / rpc);
+    const int cap = (m->sm_count > 0 ? m->sm_count : 148) * 8;
+    if (grid > cap) grid = cap;
+    if (grid > RS_RED_CTAS) grid = RS_RED_CTAS;
+    const int nq_out = nq;    // rows of `out`; the partial sums may hold more quantities than asked for
+    if (vec == 1)
+        block_reduce_kernel<1, 3, false><<<grid, RED_THREADS, 0, st>>>(a, b, eps, lanes, m->np, ncol, tshift, partial), nq = 3;
+    else if (mode == 1)
+        block_reduce_kernel<2, 2, true><<<grid, RED_THREADS, 0, st>>>(a, b, nullptr, lanes, m->np, ncol, tshift, partial), nq = 2;
+    else if (nq == 1)
+        block_reduce_kernel<2, 1, false><<<grid, RED_THREADS, 0, st>>>(a, b, nullptr, lanes, m->np, ncol, tshift, partial);
+    else
+        block_reduce_kernel<2, 3, false><<<grid, RED_THREADS, 0, st>>>(a, b, eps, lanes, m->np, ncol, tshift, partial), nq = 3;
+    RS_CUDA_TRY(cudaGetLastError());
+    block_reduce_final_kernel<<<1, 256, 0, st>>>(partial, grid, nq, nq_out, ncol, lanes, mode, out);
+    RS_CUDA_TRY(cudaGetLastError());
+    return RS_OK;
+}
+
+rs_status rs_launch_block_axpy(const rs_mesh *m, const double *alpha, const double *x, double *y, int ncol, int lanes, cudaStream_t st)
+{
+    const int cap = (m->sm_count > 0 ? m->sm_count : 148) * 16;
+    if (ncol == 1) {
+        int grid = (int)((m->np + 255) / 256);
+        block_axpy1_kernel<<<grid > cap ? cap : grid, 256, 0, st>>>(alpha, x, y, m->np);
+    } else {
+        const int64_t n2 = m->np * (int64_t)(ncol / 2);
+        int grid = (int)((n2 + 255) / 256 > cap ? cap : (n2 + 255) / 256);
+        if (lanes == 2)
+            block_axpy_kernel<true><<<grid, 256, 0, st>>>(alpha, x, y, n2, ncol / 2);
+        else
+            block_axpy_kernel<false><<<grid, 256, 0, st>>>(alpha, x, y, n2, ncol / 2);
+    }
+    RS_CUDA_TRY(cudaGetLastError());
+    return RS_OK;
+}

@@ -90,7 +90,9 @@ struct rs_mesh {
     std::map<std::pair<int, int>, rs_sweep_costs> sweep_costs;       // measured step costs, if autotuned
     std::vector<rs_sweep_map_cache> map_cache;                       // tensor maps per psi buffer (blocks wider than 16 columns)
     rs_sweep_options opt = {32, 1 << 20, 0, 0, 3, 3};                // rs_mesh_set_sweep_options
+    double *d_red = nullptr;                                         // per-CTA partial sums of the block reductions (rs_blas.cu)
 };
+constexpr int RS_RED_CTAS = 1184;                                    // at most 8 reduction CTAs per SM
 
 void rs_set_error(const std::string &msg);
 rs_status rs_fail(rs_status st, const std::string &msg);
@@ -135,3 +137,10 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
 rs_status rs_sweep_prepare(const rs_mesh *m, int n, int ncol);   // build + upload the tables now
 rs_status rs_sweep_autotune(const rs_mesh *m, int n, const rs_weights &w, const double *vloc, const double *psi, double *hpsi,
                             int ncol, cudaStream_t st);
+
+// rs_blas.cu: block operations between orbitals (f1)
+rs_status rs_launch_block_reduce(const rs_mesh *m, const double *a, const double *b, const double *eps, int ncol, int lanes,
+                                 int nq, int mode, double *out, cudaStream_t st);
+rs_status rs_launch_block_axpy(const rs_mesh *m, const double *alpha, const double *x, double *y, int ncol, int lanes,
+                               cudaStream_t st);
+rs_status rs_reduce_scratch(const rs_mesh *m, double **out);

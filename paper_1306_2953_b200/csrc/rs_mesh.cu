@@ -197,6 +197,7 @@ extern "C" rs_status rs_mesh_destroy(rs_mesh *m)
         for (int n = 0; n <= RS_MAX_FD_ORDER; ++n)
             if (m->d_map[n]) cudaFree(m->d_map[n]);
         rs_sweep_free(m);
+        cudaFree(m->d_red);
     }
     delete m;
     return RS_OK;
