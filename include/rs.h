@@ -154,11 +154,43 @@ rs_status rs_block_expectation(const rs_mesh *mesh, const void *psi_dev, const v
 rs_status rs_block_axpy(const rs_mesh *mesh, const void *alpha_dev, const void *x_dev, void *y_dev, int nst, rs_dtype dtype,
                         void *stream);
 rs_status rs_block_copy(const rs_mesh *mesh, const void *src_dev, void *dst_dev, int nst, rs_dtype dtype, void *stream);
+/* ---- overlap and subspace matrices over blocks of points (SURVEY.md 8(f) row 2; PAPER.md:203-215 eq. 5, :225-235 eq. 7)
+ *   M_dev[j][k] = sum_p conj(a[p][j]) b[p][k],  j, k < nst  (row-major [nst][nst] elements of the blocks' dtype)
+ * With b = a this is a block of the overlap matrix S (eq. 5); with b = H a (rs_hamiltonian_apply's output) a block of the
+ * subspace Hamiltonian h (eq. 7).  The block layout (all orbital coefficients of a point contiguous) is the paper's
+ * "block-of-points" array, so the rank-k update runs on the blocks as they are: a hand-written fp64 tensor-core
+ * (DMMA) contraction, deterministic (per-CTA partial matrices added in a fixed order by a second kernel).  Both blocks
+ * have width nst.  Same stream rule as the reductions above.                                                    */
+rs_status rs_block_overlap(const rs_mesh *mesh, const void *a_dev, const void *b_dev, int nst, rs_dtype dtype, void *M_dev,
+                           void *stream);
 /* rs_hamiltonian_apply plus, from the same call, sums_dev = the three rows of rs_block_expectation(psi, H psi, eps):
  * what one eigensolver step needs per orbital (Rayleigh quotient numerator and denominator, residual norm).        */
 rs_status rs_hamiltonian_apply_ex(const rs_mesh *mesh, int fd_order, const double *coeffs_host, const double *vloc_dev,
                                   const void *psi_dev, void *hpsi_dev, int nst, rs_dtype dtype, void *stream,
                                   const double *eps_dev, double *sums_dev);
+
+/* ---- non-local potential (sec. V.C, eq. 4 at :181) -------------------------------
+ *   hpsi[r][j] += sum_A sum_lm gamma^A_lm(r - R_A) * h^3 sum_{r' in sphere A} gamma^A_lm(r' - R_A) psi[r'][j]
+ * in the paper's two parts: the projection integrals are computed and stored, then multiplied by the projectors and
+ * added, atoms grouped into colours whose spheres share no mesh point so that each colour is one race-free launch
+ * (Fig. 11).  The sphere of atom A is the closed ball |r - R_A| <= rc restricted to the mesh.
+ * The projector VALUES are an input (pseudopotential data, real): after rs_nonlocal_create the caller reads each atom's
+ * sphere points (rs_nonlocal_sphere_size / rs_nonlocal_get_sphere: mesh indices, ascending), samples its nlm projectors
+ * there and hands them over with rs_nonlocal_set_projectors (host [npts_A][nlm]).  nlm <= 16 (l_max = 3).
+ * rs_nonlocal_apply ACCUMULATES into hpsi (call it after rs_hamiltonian_apply); asynchronous on `stream`; the first
+ * call uploads the tables (rs_nonlocal_prepare does that ahead of time); deterministic (fixed-order sums, no atomics).
+ * The handle keeps per-call scratch: one apply at a time per handle.  The mesh must outlive the handle.           */
+typedef struct rs_nonlocal rs_nonlocal; /* opaque */
+rs_status rs_nonlocal_create(const rs_mesh *mesh, const double *centers_host, int natoms, double rc, int nlm,
+                             rs_nonlocal **out);
+rs_status rs_nonlocal_destroy(rs_nonlocal *nl);
+int64_t rs_nonlocal_sphere_size(const rs_nonlocal *nl, int atom);                          /* -1 on bad arguments */
+rs_status rs_nonlocal_get_sphere(const rs_nonlocal *nl, int atom, int32_t *mesh_index_host);
+rs_status rs_nonlocal_set_projectors(rs_nonlocal *nl, int atom, const double *gamma_host);
+int rs_nonlocal_ncolors(const rs_nonlocal *nl);
+rs_status rs_nonlocal_get_colors(const rs_nonlocal *nl, int32_t *color_host /*[natoms]*/);
+rs_status rs_nonlocal_prepare(rs_nonlocal *nl);
+rs_status rs_nonlocal_apply(rs_nonlocal *nl, const void *psi_dev, void *hpsi_dev, int nst, rs_dtype dtype, void *stream);
 
 /* Once per (mesh, fd_order, nst, dtype), before the first apply: build and upload the neighbour structure the chosen
  * kernel needs (plain table for the gather kernel, per-plane records for the plane-sweep kernel).  May allocate and

@@ -37,7 +37,9 @@ EXPORTS = (
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
     "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version",
     "rs_sweep_options_default", "rs_mesh_set_sweep_options", "rs_hamiltonian_prepare",
-    "rs_block_dot", "rs_block_expectation", "rs_block_axpy", "rs_block_copy", "rs_hamiltonian_apply_ex",
+    "rs_block_dot", "rs_block_expectation", "rs_block_axpy", "rs_block_copy", "rs_hamiltonian_apply_ex", "rs_block_overlap",
+    "rs_nonlocal_create", "rs_nonlocal_destroy", "rs_nonlocal_sphere_size", "rs_nonlocal_get_sphere", "rs_nonlocal_set_projectors",
+    "rs_nonlocal_ncolors", "rs_nonlocal_get_colors", "rs_nonlocal_prepare", "rs_nonlocal_apply",
     "rs_workspace_create", "rs_workspace_destroy", "rs_workspace_bytes", "rs_hamiltonian_apply_states_stream",
     "rs_sweep_selfcheck", "rs_sweep_stats", "rs_hamiltonian_autotune",
 )
@@ -87,6 +89,17 @@ def _load() -> C.CDLL:
     L.rs_block_dot.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp, vp]
     L.rs_block_expectation.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, vp, vp]
     L.rs_block_axpy.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, vp]
+    L.rs_nonlocal_create.argtypes = [vp, dp, C.c_int, C.c_double, C.c_int, C.POINTER(vp)]
+    L.rs_nonlocal_destroy.argtypes = [vp]
+    L.rs_nonlocal_sphere_size.argtypes = [vp, C.c_int]
+    L.rs_nonlocal_sphere_size.restype = C.c_int64
+    L.rs_nonlocal_get_sphere.argtypes = [vp, C.c_int, i32p]
+    L.rs_nonlocal_set_projectors.argtypes = [vp, C.c_int, dp]
+    L.rs_nonlocal_ncolors.argtypes = [vp]
+    L.rs_nonlocal_get_colors.argtypes = [vp, i32p]
+    L.rs_nonlocal_prepare.argtypes = [vp]
+    L.rs_nonlocal_apply.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp]
+    L.rs_block_overlap.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp, vp]
     L.rs_block_copy.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp]
     L.rs_hamiltonian_apply_ex.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int, C.c_int, vp, vp, vp]
     L.rs_workspace_create.argtypes = [vp, C.c_int, C.c_int, C.c_int64, C.c_int, C.POINTER(vp)]
@@ -330,6 +343,11 @@ def rs_block_axpy(mesh: Mesh, alpha, x, y, nst: int, stream=None) -> None:
     _check(_lib.rs_block_axpy(mesh.handle, _ptr(alpha), _ptr(x), _ptr(y), nst, _dtype_of(x), _stream(stream)))
 
 
+def rs_block_overlap(mesh: Mesh, a, b, nst: int, M, stream=None) -> None:
+    """M[j][k] = sum_p conj(a[p][j]) b[p][k] (device tensors; M: [nst][nst] of the blocks' dtype): eqs. 5 / 7."""
+    _check(_lib.rs_block_overlap(mesh.handle, _ptr(a), _ptr(b), nst, _dtype_of(a), _ptr(M), _stream(stream)))
+
+
 def rs_block_copy(mesh: Mesh, src, dst, nst: int, stream=None) -> None:
     _check(_lib.rs_block_copy(mesh.handle, _ptr(src), _ptr(dst), nst, _dtype_of(src), _stream(stream)))
 
@@ -341,6 +359,57 @@ def rs_hamiltonian_apply_ex(mesh: Mesh, fd_order: int, coeffs, vloc, psi, hpsi, 
         raise RsError(RS_ERR_INVALID_ARG, "coeffs must hold c_0..c_n")
     _check(_lib.rs_hamiltonian_apply_ex(mesh.handle, fd_order, _dptr(c), _ptr(vloc), _ptr(psi), _ptr(hpsi), nst,
                                         _dtype_of(psi), _stream(stream), _ptr(eps) if eps is not None else None, _ptr(sums)))
+
+
+class NonLocal:
+    """Owner of an rs_nonlocal handle (projector spheres, colouring, device tables); keeps its mesh alive."""
+
+    def __init__(self, mesh: Mesh, centers, rc: float, nlm: int):
+        c = np.ascontiguousarray(centers, dtype=np.float64).reshape(-1, 3)
+        out = C.c_void_p()
+        _check(_lib.rs_nonlocal_create(mesh.handle, _dptr(c), c.shape[0], rc, nlm, C.byref(out)))
+        self._h, self.mesh, self.natoms, self.nlm = out, mesh, c.shape[0], nlm
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h and _lib is not None:
+            _lib.rs_nonlocal_destroy(h)
+
+    def sphere(self, atom: int) -> np.ndarray:
+        """mesh indices (ascending) of the atom's sphere points = the row order of its projector table."""
+        n = int(_lib.rs_nonlocal_sphere_size(self._h, atom))
+        if n < 0:
+            raise RsError(RS_ERR_INVALID_ARG, "bad atom index")
+        idx = np.empty(n, dtype=np.int32)
+        _check(_lib.rs_nonlocal_get_sphere(self._h, atom, idx.ctypes.data_as(C.POINTER(C.c_int32))))
+        return idx
+
+    def set_projectors(self, atom: int, gamma) -> None:
+        g = np.ascontiguousarray(gamma, dtype=np.float64)
+        if g.shape != (int(_lib.rs_nonlocal_sphere_size(self._h, atom)), self.nlm):
+            raise RsError(RS_ERR_INVALID_ARG, "projector table must be [sphere points][nlm]")
+        _check(_lib.rs_nonlocal_set_projectors(self._h, atom, _dptr(g)))
+
+    @property
+    def ncolors(self) -> int:
+        return int(_lib.rs_nonlocal_ncolors(self._h))
+
+    def colors(self) -> np.ndarray:
+        c = np.empty(self.natoms, dtype=np.int32)
+        _check(_lib.rs_nonlocal_get_colors(self._h, c.ctypes.data_as(C.POINTER(C.c_int32))))
+        return c
+
+    def prepare(self) -> None:
+        _check(_lib.rs_nonlocal_prepare(self._h))
+
+
+def rs_nonlocal_create(mesh: Mesh, centers, rc: float, nlm: int) -> NonLocal:
+    return NonLocal(mesh, centers, rc, nlm)
+
+
+def rs_nonlocal_apply(nl: NonLocal, psi, hpsi, nst: int, stream=None) -> None:
+    """hpsi += V_nl psi on one block (eq. 4 of the paper); device tensors."""
+    _check(_lib.rs_nonlocal_apply(nl._h, _ptr(psi), _ptr(hpsi), nst, _dtype_of(psi), _stream(stream)))
 
 
 class Workspace:

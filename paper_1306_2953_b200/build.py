@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 SO = os.path.join(HERE, "librs.so")
 
-SOURCES = ["rs_api.cu", "rs_mesh.cu", "rs_kernels.cu", "rs_sweep.cu", "rs_blas.cu"]
+SOURCES = ["rs_api.cu", "rs_mesh.cu", "rs_kernels.cu", "rs_sweep.cu", "rs_blas.cu", "rs_overlap.cu", "rs_nonlocal.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",

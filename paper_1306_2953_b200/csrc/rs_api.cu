@@ -125,6 +125,18 @@ extern "C" rs_status rs_block_copy(const rs_mesh *m, const void *src, void *dst,
     return RS_OK;
 }
 
+// ---- f2: overlap / subspace matrices over blocks of points (eqs. 5 and 7) -----------------------
+extern "C" rs_status rs_block_overlap(const rs_mesh *m, const void *a, const void *b, int nst, rs_dtype dtype, void *M_dev, void *stream)
+{
+    rs_status st = check_blocks(m, a, b, nst, dtype, "rs_block_overlap");
+    if (st != RS_OK) return st;
+    if (!M_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_overlap: null output");
+    const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
+    if (nst * lanes == 1)   // a single real column: the 1 x 1 matrix is the dot product
+        return rs_launch_block_reduce(m, (const double *)a, (const double *)b, nullptr, 1, 1, 1, 0, (double *)M_dev, (cudaStream_t)stream);
+    return rs_launch_overlap(m, (const double *)a, (const double *)b, nst * lanes, lanes, (double *)M_dev, (cudaStream_t)stream);
+}
+
 // H psi and, from the same call, the per-orbital sums an eigensolver step needs.  The gather kernel and (for now) the
 // plane-sweep kernel form the sums in a second streaming kernel over psi and H psi (one extra read of both blocks).
 extern "C" rs_status rs_hamiltonian_apply_ex(const rs_mesh *m, int n, const double *coeffs, const double *vloc, const void *psi,
@@ -374,10 +386,12 @@ extern "C" rs_status rs_hamiltonian_prepare(const rs_mesh *m, int n, int nst, rs
     if (resolve_kernel(m, n, ncol, RS_KERNEL_AUTO) == RS_KERNEL_SWEEP) {
         double *scr = nullptr;
         rs_status s2 = rs_reduce_scratch(m, &scr);
+        if (s2 == RS_OK) s2 = rs_overlap_scratch(m, &scr);
         return s2 != RS_OK ? s2 : rs_sweep_prepare(m, n, ncol);
     }
     double *scratch = nullptr;
     rs_status st = rs_reduce_scratch(m, &scratch);   // the block reductions' per-CTA partial sums
+    if (st == RS_OK) st = rs_overlap_scratch(m, &scratch);
     if (st != RS_OK) return st;
     const int32_t *d_map = nullptr;
     return rs_mesh_device_map(m, n, &d_map);

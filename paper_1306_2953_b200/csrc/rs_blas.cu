@@ -66,28 +66,36 @@ __global__ void __launch_bounds__(RED_THREADS) block_reduce_kernel(const double 
     }
 }
 
-// out[q][j] = sum over CTAs (in order) and over the orbital's lanes of partial[cta][q][j*lanes + l]; mode 1 (complex dot):
-// out[j] = (re, im) with re = q0 over both lanes, im = the extra sum kept in the im column of the last quantity.
-__global__ void block_reduce_final_kernel(const double *__restrict__ partial, int nctas, int nq, int nq_out, int ncol, int lanes,
-                                          int mode, double *__restrict__ out)
+// One warp per output: lane l adds the slots of CTAs l, l + 32, ... in that order, then a fixed butterfly adds the 32 lane
+// sums: the same bits on every run.  mode 0: out[q][j] = sum over CTAs and over the orbital's lanes of partial[cta][q][j*lanes + l];
+// mode 1 (complex dot, nq == 2): out[j] = (re, im), re = q0 over both lanes, im = the cross terms kept in the im column of q1.
+__global__ void __launch_bounds__(256) block_reduce_final_kernel(const double *__restrict__ partial, int nctas, int nq, int nq_out,
+                                                                 int ncol, int lanes, int mode, double *__restrict__ out)
 {
-    const int nst = ncol / lanes;
-    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nq_out * nst; idx += gridDim.x * blockDim.x) {
-        const int q = idx / nst, j = idx % nst;
-        if (mode == 1) {                       // complex dot: nq == 2 here (q0 = products, q1 = cross terms)
-            if (q != 0) continue;
-            double re = 0.0, im = 0.0;
-            for (int c = 0; c < nctas; ++c) {
-                re += partial[((size_t)c * 2 + 0) * ncol + 2 * j] + partial[((size_t)c * 2 + 0) * ncol + 2 * j + 1];
-                im += partial[((size_t)c * 2 + 1) * ncol + 2 * j + 1];
-            }
-            out[2 * j] = re, out[2 * j + 1] = im;
-        } else {
-            double s = 0.0;
-            for (int c = 0; c < nctas; ++c)
-                for (int l = 0; l < lanes; ++l) s += partial[((size_t)c * nq + q) * ncol + j * lanes + l];
-            out[(size_t)q * nst + j] = s;
+    const int nst = ncol / lanes, lane = threadIdx.x & 31;
+    const int idx = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (idx >= nq_out * nst) return;
+    const int q = idx / nst, j = idx % nst;
+    double s0 = 0.0, s1 = 0.0;
+    if (mode == 1) {
+        for (int c = lane; c < nctas; c += 32) {
+            s0 += partial[((size_t)c * 2 + 0) * ncol + 2 * j] + partial[((size_t)c * 2 + 0) * ncol + 2 * j + 1];
+            s1 += partial[((size_t)c * 2 + 1) * ncol + 2 * j + 1];
         }
+    } else {
+        for (int c = lane; c < nctas; c += 32)
+            for (int l = 0; l < lanes; ++l) s0 += partial[((size_t)c * nq + q) * ncol + j * lanes + l];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    }
+    if (lane == 0) {
+        if (mode == 1)
+            out[2 * j] = s0, out[2 * j + 1] = s1;
+        else
+            out[(size_t)q * nst + j] = s0;
     }
 }
 
@@ -161,7 +169,7 @@ rs_status rs_launch_block_reduce(const rs_mesh *m, const double *a, const double
     else
         block_reduce_kernel<2, 3, false><<<grid, RED_THREADS, 0, st>>>(a, b, eps, lanes, m->np, ncol, tshift, partial), nq = 3;
     RS_CUDA_TRY(cudaGetLastError());
-    block_reduce_final_kernel<<<1, 256, 0, st>>>(partial, grid, nq, nq_out, ncol, lanes, mode, out);
+    block_reduce_final_kernel<<<(nq_out * (ncol / lanes) * 32 + 255) / 256, 256, 0, st>>>(partial, grid, nq, nq_out, ncol, lanes, mode, out);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
 }

@@ -91,6 +91,7 @@ struct rs_mesh {
     std::vector<rs_sweep_map_cache> map_cache;                       // tensor maps per psi buffer (blocks wider than 16 columns)
     rs_sweep_options opt = {32, 1 << 20, 0, 0, 3, 3};                // rs_mesh_set_sweep_options
     double *d_red = nullptr;                                         // per-CTA partial sums of the block reductions (rs_blas.cu)
+    double *d_ovl = nullptr;                                         // per-CTA partial matrices of rs_block_overlap (rs_overlap.cu)
 };
 constexpr int RS_RED_CTAS = 1184;                                    // at most 8 reduction CTAs per SM
 
@@ -144,3 +145,7 @@ rs_status rs_launch_block_reduce(const rs_mesh *m, const double *a, const double
 rs_status rs_launch_block_axpy(const rs_mesh *m, const double *alpha, const double *x, double *y, int ncol, int lanes,
                                cudaStream_t st);
 rs_status rs_reduce_scratch(const rs_mesh *m, double **out);
+
+// rs_overlap.cu: overlap / subspace matrices (f2)
+rs_status rs_launch_overlap(const rs_mesh *m, const double *x, const double *y, int cr, int lanes, double *M, cudaStream_t st);
+rs_status rs_overlap_scratch(const rs_mesh *m, double **out);

@@ -198,6 +198,7 @@ extern "C" rs_status rs_mesh_destroy(rs_mesh *m)
             if (m->d_map[n]) cudaFree(m->d_map[n]);
         rs_sweep_free(m);
         cudaFree(m->d_red);
+        cudaFree(m->d_ovl);
     }
     delete m;
     return RS_OK;

@@ -124,3 +124,125 @@ def test_apply_ex_sums_match_the_oracle(B, is_complex):
     assert (np.abs(s[1] - n_o) <= 1e-12 * n_o).all()
     r2 = np.real(oracle.block_dot(r, r))
     assert (np.abs(s[2] - r2) <= 1e-11 * np.linalg.norm(o, axis=1) ** 2).all()
+
+
+# ---- f2 ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("is_complex", [False, True])
+@pytest.mark.parametrize("B,nst", [(1, 1), (2, 2), (4, 3), (8, 8), (16, 13), (32, 32), (64, 64)])
+def test_block_overlap_matches_the_oracle(B, nst, is_complex):
+    """S-type (b = a, same buffer) and rectangular-type (b != a) blocks on config 1 (262 k points: ~2000 point tiles with a
+    ragged last one, every kernel shape 8..128 real columns); the oracle's triple loop is O(nst^2 np), so the widest
+    cases compare a seeded sample of matrix rows."""
+    import torch
+
+    p = problem(1)
+    a = rand_orbitals(3 * B, nst, p.np, is_complex)
+    b = rand_orbitals(3 * B + 1, nst, p.np, is_complex)
+    A, Bk = to_block(p, a, B), to_block(p, b, B)
+    na, nb = np.linalg.norm(a, axis=1), np.linalg.norm(b, axis=1)
+    rows = list(range(nst)) if nst <= 16 else sorted(np.random.default_rng(B).choice(nst, 6, replace=False).tolist())
+    for X, Y, x, y, ny in ((A, A, a, a, na), (A, Bk, a, b, nb)):
+        M = torch.full((B, B), 7.0, dtype=A.dtype, device="cuda")
+        rs.rs_block_overlap(p.mesh, X, Y, B, M)
+        g = M.cpu().numpy()
+        o = oracle.overlap(x[rows], y)
+        assert (np.abs(g[rows][:, :nst] - o) <= 1e-12 * np.outer(na[rows], ny)).all()
+        assert np.all(g[nst:] == 0) and np.all(g[:, nst:] == 0)          # padding columns
+        if X is Y:
+            assert np.abs(g - np.conj(g.T)).max() <= 1e-12 * (na.max() ** 2)
+        M2 = torch.empty_like(M)
+        rs.rs_block_overlap(p.mesh, X, Y, B, M2)
+        assert torch.equal(M, M2)                                       # deterministic
+
+
+def test_subspace_hamiltonian_of_plane_waves_is_diagonal():
+    """eq. 7 end to end on the CUDA path: h = Psi^dagger (H Psi) for plane waves on the periodic box = N^3 diag(lambda(q))."""
+    import math
+    import torch
+
+    n, h, N, v0 = 4, 0.25, 16, 0.3
+    p = Problem(None, None, None, h, max_n=4, box=(N, N, N), periodic=True)
+    p.v_canon[:] = v0
+    p.v_mesh[:] = v0
+    ijk = p.omesh.ijk().astype(np.float64)
+    ms = [(1, 2, 3), (2, 0, 5), (0, 0, 0), (3, 3, 1)]
+    qs = [[2 * math.pi * ma / (N * h) for ma in m] for m in ms]
+    psi = np.stack([np.exp(1j * sum(q[a] * ijk[:, a] * h for a in range(3))) for q in qs])
+    B = 4
+    blk = to_block(p, psi, B)
+    hblk = torch.empty_like(blk)
+    c = np.array([-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560])
+    rs.rs_hamiltonian_apply(p.mesh, n, c, torch.from_numpy(p.v_mesh).cuda(), blk, hblk, B)
+    S = torch.empty((B, B), dtype=torch.complex128, device="cuda")
+    Hm = torch.empty_like(S)
+    rs.rs_block_overlap(p.mesh, blk, blk, B, S)
+    rs.rs_block_overlap(p.mesh, blk, hblk, B, Hm)
+    lam = np.array([-0.5 * sum((c[0] + 2 * sum(c[k] * math.cos(k * q[a] * h) for k in range(1, n + 1))) / h ** 2 for a in range(3)) + v0
+                    for q in qs])
+    assert np.abs(S.cpu().numpy() - N ** 3 * np.eye(B)).max() <= 1e-12 * N ** 3
+    assert np.abs(Hm.cpu().numpy() - N ** 3 * np.diag(lam)).max() <= 1e-12 * N ** 3 * np.abs(lam).max()
+
+
+# ---- f3 ----------------------------------------------------------------------------------------------------------
+def make_nonlocal(p, centers, rc, lmax, sigma=0.7):
+    """The same INPUT (synthetic.projector_values) on both sides: the library samples it at the sphere points it
+    publishes, the oracle at its own; the two point sets are compared first."""
+    nlm = (lmax + 1) ** 2
+    nl = rs.rs_nonlocal_create(p.mesh, centers, rc, nlm)
+    h = p.mesh.spacing
+    for A in range(len(centers)):
+        idx = nl.sphere(A)
+        assert np.array_equal(np.sort(p.rank[idx]), oracle.sphere_points(p.omesh, centers[A], rc))
+        nl.set_projectors(A, synthetic.projector_values(p.ijk[idx].astype(np.float64) * h - centers[A], lmax, sigma))
+    proj = oracle.make_projectors(p.omesh, centers, rc, lambda x: synthetic.projector_values(x, lmax, sigma))
+    return nl, proj
+
+
+@pytest.mark.parametrize("B,nst,is_complex,lmax", [(1, 1, False, 0), (4, 3, False, 1), (16, 16, False, 1), (16, 9, True, 1),
+                                                   (32, 32, False, 2), (64, 64, False, 1), (64, 40, True, 0)])
+def test_nonlocal_apply_matches_the_oracle(B, nst, is_complex, lmax):
+    """eq. 4 on config 1: 12 atoms with overlapping projector spheres (several colours), accumulated into an existing H psi."""
+    import torch
+
+    p = problem(1)
+    centers = p.cfg.centers
+    key = ("nl", lmax)
+    if key not in _cache:
+        _cache[key] = make_nonlocal(p, centers, 2.0, lmax)
+    nl, proj = _cache[key]
+    assert nl.ncolors >= 2
+    psi = rand_orbitals(40 + B, nst, p.np, is_complex)
+    base = rand_orbitals(41 + B, nst, p.np, is_complex)
+    blk, hblk = to_block(p, psi, B), to_block(p, base, B)
+    rs.rs_nonlocal_apply(nl, blk, hblk, B)
+    g = from_block(p, hblk, nst)
+    o = oracle.nonlocal_apply(p.omesh, proj, psi, base)
+    vn = oracle.nonlocal_apply(p.omesh, proj, np.abs(psi.real) + (np.abs(psi.imag) if is_complex else 0.0))   # no cancellation: scale
+    assert np.abs(g - o).max() <= 1e-12 * np.abs(o).max()
+    assert (np.abs(g - o) <= 1e-12 * (np.abs(vn).max() + np.abs(base))).all()
+    hb2 = to_block(p, base, B)
+    rs.rs_nonlocal_apply(nl, blk, hb2, B)
+    assert torch.equal(hblk, hb2)                                   # deterministic
+    assert torch.all(hblk[p.np] == 0)
+
+
+def test_full_hamiltonian_with_nonlocal_term_is_hermitian_on_gpu():
+    """H = -1/2 Lap + V_loc + V_nl through the CUDA path: <phi|H psi> = <H phi|psi> (all three terms)."""
+    import torch
+
+    p = problem(1)
+    key = ("nl", 1)
+    if key not in _cache:
+        _cache[key] = make_nonlocal(p, p.cfg.centers, 2.0, 1)
+    nl, _ = _cache[key]
+    B = 2
+    f = rand_orbitals(5, 2, p.np, True)
+    blk = to_block(p, f, B)
+    hblk = torch.empty_like(blk)
+    rs.rs_hamiltonian_apply(p.mesh, 4, oracle.fd_coeffs(4), torch.from_numpy(p.v_mesh).cuda(), blk, hblk, B)
+    rs.rs_nonlocal_apply(nl, blk, hblk, B)
+    M = torch.empty((B, B), dtype=torch.complex128, device="cuda")
+    rs.rs_block_overlap(p.mesh, blk, hblk, B, M)                     # M[0][1] = <phi|H psi>, M[1][0] = <psi|H phi>
+    m = M.cpu().numpy()
+    hp = from_block(p, hblk, 2)
+    assert abs(m[0, 1] - np.conj(m[1, 0])) <= 1e-13 * np.linalg.norm(f[0]) * np.linalg.norm(hp[1])

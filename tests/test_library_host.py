@@ -279,3 +279,37 @@ def test_sweep_records_on_random_sparse_clusters(seed):
         for nst, planes, nctas in ((16, int(rng.integers(4, 40)), int(rng.integers(1, 200))), (32, 1 << 20, 148)):
             st = rs.rs_sweep_selfcheck(mesh, n, nst, rs.RS_REAL64, planes, nctas)
             assert st["records"] > 0
+
+
+# ---- f3: non-local potential, host side (spheres, colouring) -- no device needed ------------------------------------
+def test_nonlocal_spheres_equal_the_oracles_and_colours_are_race_free():
+    """The library's projector spheres (closed ball on the mesh) are the oracle's point sets, and no two atoms of one
+    colour share a mesh point ("groups whose spheres do not overlap")."""
+    cfg = synthetic.config(1)                                   # 12 centres, heavily overlapping spheres at rc = 2.0
+    mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, 4)
+    om = oracle.mesh_from_spheres(cfg.centers, cfg.radius, cfg.spacing)
+    rank = synthetic.canonical_rank(mesh.points())
+    rc = 2.0
+    nl = rs.rs_nonlocal_create(mesh, cfg.centers, rc, 4)
+    sets = []
+    for A in range(cfg.centers.shape[0]):
+        idx = nl.sphere(A)
+        assert np.all(np.diff(idx) > 0)
+        assert np.array_equal(np.sort(rank[idx]), oracle.sphere_points(om, cfg.centers[A], rc))
+        sets.append(set(idx.tolist()))
+    col = nl.colors()
+    assert col.min() == 0 and col.max() + 1 == nl.ncolors and nl.ncolors >= 2
+    for A in range(len(sets)):
+        for Bq in range(A):
+            if col[A] == col[Bq]:
+                assert not (sets[A] & sets[Bq]), (A, Bq)
+    # greedy: every atom of colour c > 0 conflicts with some atom of every lower colour
+    for A in range(len(sets)):
+        for c in range(col[A]):
+            assert any(col[Bq] == c and (sets[A] & sets[Bq]) for Bq in range(len(sets)))
+    # far-apart atoms: one colour; a sphere outside the mesh: empty
+    far = rs.rs_nonlocal_create(mesh, np.array([[0.0, 0.0, 0.0], [100.0, 0.0, 0.0]]), 1.0, 1)
+    assert far.ncolors == 1 and far.sphere(1).size == 0 and far.sphere(0).size > 0
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_nonlocal_create(mesh, cfg.centers, rc, 17)
+    assert e.value.status == rs.RS_ERR_INVALID_ARG
