@@ -65,7 +65,9 @@ typedef enum { RS_REAL64 = 0, RS_COMPLEX128 = 1 } rs_dtype;
  * sequence of small parallelepipedic grids").  Results do not depend on it beyond rounding order. */
 typedef enum {
     RS_ORDER_BRICK = 0, /* the paper's 4x4x4 bricks, brick after brick (gather kernel only; ablation of Fig. 8) */
-    RS_ORDER_LEX = 1    /* lexicographic (i, j, k), k fastest (default; what the plane-sweep kernel streams)    */
+    RS_ORDER_LEX = 1,   /* lexicographic (i, j, k), k fastest (default; what the plane-sweep kernel streams)    */
+    RS_ORDER_TILE = 2   /* 16 x 16 tiles of the (j, k) plane, each marched along i: a tile's points of one plane are
+                           consecutive (gather kernel only; ordering study)                          */
 } rs_ordering;
 
 /* Kernel selection for rs_hamiltonian_apply_v (tests and ablations; results agree to rounding). */

@@ -23,7 +23,7 @@ from . import build as _build
 
 RS_OK, RS_ERR_INVALID_ARG, RS_ERR_ALLOC, RS_ERR_CUDA, RS_ERR_UNSUPPORTED = range(5)
 RS_REAL64, RS_COMPLEX128 = 0, 1
-RS_ORDER_BRICK, RS_ORDER_LEX = 0, 1
+RS_ORDER_BRICK, RS_ORDER_LEX, RS_ORDER_TILE = 0, 1, 2
 RS_KERNEL_AUTO, RS_KERNEL_GATHER, RS_KERNEL_SWEEP = 0, 1, 2
 RS_MAX_FD_ORDER = 8
 RS_MAX_BLOCK = 64

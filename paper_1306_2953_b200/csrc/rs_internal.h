@@ -23,8 +23,9 @@ constexpr int RS_BRICK_PTS = RS_BRICK * RS_BRICK * RS_BRICK;  // 64 points
 //   fill[18 (+2 pad)]      bitmap over the stage's [24][24] slots: slots to clear (lattice point outside the mesh
 //                          and the stage buffer does not already hold zeros there);
 //   hdr[4]                 {2 bits per warp: 0 no mesh point in the warp's 4 x 8 region, 1 centre-only, 2 full;
-//                           bit 16: output plane,  column offset of the slice,  bytes copied (1-D runs),
-//                           bytes copied (2-D tensor boxes)};
+//                           bits 16..23: entries of the clear list (0xff: walk the bitmap); bit 31: output plane,
+//                           column offset of the slice,  bytes copied (1-D runs),  bytes copied (2-D tensor boxes)};
+//   flist[64]              uint16 slots to clear, ascending = the set bits of the bitmap when there are at most 64;
 //   cidx[256]              mesh index of the tile's own points (-1: outside the mesh / not an output plane).
 #define RS_SWEEP_MAXRUN 64
 struct rs_sweep_piece {
@@ -34,7 +35,7 @@ struct rs_sweep_host {
     std::vector<int2> items;                         // per CTA: {first record, number of steps}
     std::vector<std::vector<rs_sweep_piece>> pieces; // per CTA, in execution order
     std::vector<unsigned char> recs;                 // [nrec][rec_bytes]
-    int rec_bytes = 0;                               // 608 + 4 per tile point (depends on the kernel shape)
+    int rec_bytes = 0;                               // 736 + 4 per tile point (depends on the kernel shape)
     std::vector<int32_t> rec_cell;                   // per record: tile * nx + x of an output plane, -1 for a halo step
     int64_t nrec = 0;
     std::vector<double> load;                        // modelled load per CTA

@@ -46,6 +46,19 @@ static void enumerate_points(rs_mesh *m, const std::vector<uint8_t> &in)
         m->np = count;
         return;
     }
+    if (m->ordering == RS_ORDER_TILE) {
+        // tile columns: the (y, z) plane is cut into 16 x 16 tiles; a tile's points of plane x are consecutive, plane after
+        // plane (the order in which the plane-sweep kernel visits the mesh; ordering study)
+        constexpr int T = 16;
+        for (int ty = 0; ty < ny; ty += T)
+            for (int tz = 0; tz < nz; tz += T)
+                for (int ix = 0; ix < nx; ++ix)
+                    for (int iy = ty; iy < std::min(ny, ty + T); ++iy)
+                        for (int iz = tz; iz < std::min(nz, tz + T); ++iz)
+                            if (in[dense_index(m, ix, iy, iz)]) push(ix, iy, iz);
+        m->np = count;
+        return;
+    }
     // paper's enumeration: brick after brick, points inside a brick in (x, y, z) order
     const int nb[3] = {m->dims[0] / RS_BRICK, m->dims[1] / RS_BRICK, m->dims[2] / RS_BRICK};
     m->nbricks = 0;
@@ -101,7 +114,7 @@ extern "C" rs_status rs_mesh_create_ordered(const double *centers, int nc, doubl
                                             int max_fd_order, rs_ordering ordering, rs_mesh **out)
 {
     if (!centers || !out || nc < 1 || !(radius > 0.0) || !(spacing > 0.0) || max_fd_order < 1 ||
-        max_fd_order > RS_MAX_FD_ORDER || (ordering != RS_ORDER_BRICK && ordering != RS_ORDER_LEX))
+        max_fd_order > RS_MAX_FD_ORDER || (ordering != RS_ORDER_BRICK && ordering != RS_ORDER_LEX && ordering != RS_ORDER_TILE))
         return rs_fail(RS_ERR_INVALID_ARG, "rs_mesh_create: bad argument");
     *out = nullptr;
     rs_mesh *m = new (std::nothrow) rs_mesh;
@@ -168,7 +181,7 @@ extern "C" rs_status rs_mesh_create_box(int nx, int ny, int nz, double spacing, 
                                         rs_ordering ordering, rs_mesh **out)
 {
     if (!out || nx < 1 || ny < 1 || nz < 1 || !(spacing > 0.0) || max_fd_order < 1 || max_fd_order > RS_MAX_FD_ORDER ||
-        (ordering != RS_ORDER_BRICK && ordering != RS_ORDER_LEX) || (size_t)nx * ny * nz >= ((size_t)1 << 30))
+        (ordering != RS_ORDER_BRICK && ordering != RS_ORDER_LEX && ordering != RS_ORDER_TILE) || (size_t)nx * ny * nz >= ((size_t)1 << 30))
         return rs_fail(RS_ERR_INVALID_ARG, "rs_mesh_create_box: bad argument");
     *out = nullptr;
     rs_mesh *m = new (std::nothrow) rs_mesh;

@@ -52,8 +52,11 @@ constexpr int SW_SLOT_BYTES = SW_C * 8;  // 128
 constexpr int SW_STAGES = 3;
 constexpr int SW_MAXRUN = RS_SWEEP_MAXRUN;
 constexpr int SW_TMEM_COLS = 512;
-// packed per-plane record (rs_internal.h): runs | fill bitmap | header | indices of the tile's points
-constexpr int SW_REC_RUNS = 0, SW_REC_FILL = SW_MAXRUN * 8, SW_REC_HDR = SW_REC_FILL + 80, SW_REC_CIDX = SW_REC_HDR + 16;
+// packed per-plane record (rs_internal.h): runs | fill bitmap | header | clear list | indices of the tile's points
+constexpr int SW_MAXFILL = 64;             // slots a record can list for clearing; more (a piece's first planes): the whole stage is cleared
+constexpr int SW_REC_RUNS = 0, SW_REC_FILL = SW_MAXRUN * 8, SW_REC_HDR = SW_REC_FILL + 80, SW_REC_FLIST = SW_REC_HDR + 16,
+              SW_REC_CIDX = SW_REC_FLIST + SW_MAXFILL * 2;
+constexpr uint32_t HDR_NFILL_SHIFT = 16, HDR_NFILL_WHOLE = 0xffu;   // header word 0, bits 16..23: entries of the clear list, 0xff = clear the whole stage first
 constexpr int SW_RING = 6;               // record ring of the producers
 constexpr int SW_LOOKAHEAD = 3;          // records are requested this many steps ahead (SW_RING >= SW_LOOKAHEAD + 3)
 constexpr int SW_NBOX = 6;               // tensor-map box heights 1, 2, 4, 8, 16, 24 (a run of 25..28 points takes two boxes)
@@ -263,8 +266,9 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
     const uint32_t v_off0 = (uint32_t)(((gtid >> 6) * S::WZ) * SW_SLOT_BYTES + (gtid & 63) * 8);
     const uint32_t i_off0 = (uint32_t)(((gtid >> 6) * S::WZ + S::WZ - N) * SW_SLOT_BYTES + (gtid & 63) * 4);
     constexpr uint32_t NEXT_POINT = 2 * S::WZ * SW_SLOT_BYTES;   // point gtid + 128: two corner rows further
-    int stage = group % SW_STAGES, rs = group % SW_RING;   // t mod SW_STAGES, t mod SW_RING
-    uint32_t eparity = 1, rparity = 0;                     // the first pass over the stages finds them free
+    // stage = t mod SW_STAGES, record slot rs = t mod SW_RING and the barrier parities are re-derived from t where they are
+    // needed instead of being carried: the producers run on 32 registers and a spilled V value would put the global-load
+    // latency back on the per-step path (the first pass over the stages finds them free: parity 1)
     // V and the offsets of a plane are fetched one own step ahead of their use, and nothing touches the loaded value
     // until then, so that the global-load latency is not on the per-step path (adding 3 w_0 right after the load cost
     // ~1000 clocks per step: measured 0.136 -> 0.127 ms on config 2).  The store offsets of a plane's outputs are needed N steps later, when the x arm is
@@ -290,10 +294,12 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         }
     };
     if (group < nsteps) {
-        mbar_wait(rbar0 + 8u * rs, rparity);
-        fetch_v(rs);
+        mbar_wait(rbar0 + 8u * group, 0u);
+        fetch_v(group);
     }
     for (int t = group; t < nsteps; t += G) {
+        const int stage = t % SW_STAGES, rs = t % SW_RING;
+        const uint32_t eparity = ((uint32_t)(t / SW_STAGES) & 1u) ^ 1u;
         // everything the copies need is read from the record (present: fetch_v waited for it) BEFORE the wait for
         // the stage, so that the copies leave right after the consumers release it
         const unsigned char *rp = ring + (size_t)rs * S::REC_BYTES;
@@ -305,6 +311,15 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         if (lane < SW_MAXRUN / 4) run = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
         const uint32_t len = run.y >> 16, slot = run.y & 0xffffu;
         mbar_wait(empty0 + 8u * stage, eparity);
+        const uint32_t nfill = (hdr.x >> HDR_NFILL_SHIFT) & 0xffu;
+        if (nfill == HDR_NFILL_WHOLE) {
+            // a piece's first planes: more slots to clear than the list holds -> the group clears the whole stage, and only
+            // then (group barrier) may any of its warps issue the plane's copies
+#pragma unroll 1
+            for (uint32_t o = (uint32_t)gtid * 16u; o < (uint32_t)S::STAGE_BYTES; o += 128u * 16u)
+                *reinterpret_cast<float4 *>(sg + o) = make_float4(0.f, 0.f, 0.f, 0.f);
+            named_bar_sync(2 + group, 128);
+        }
         fence_proxy_async();   // earlier generic accesses to this stage and to the record slot reused below (ordered before us by the barrier) before our async copies
         // ---- copy runs --------------------------------------------------------------------------------
         if (len) {
@@ -320,18 +335,19 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
             }
         }
         if (gtid == 0 && t + SW_LOOKAHEAD < nsteps) request_rec(t + SW_LOOKAHEAD);
-        // ---- zero fill: bit s of the record's bitmap says that slot s of the [WY][WZ] grid must be cleared.  A warp
-        //      takes every 4th word of the bitmap; a quarter-warp clears one slot with 8 conflict-free 16-byte stores ----
-#pragma unroll 1
-        for (int wd = pw; wd < (S::WY * S::WZ + 31) / 32; wd += 4) {
-            const uint32_t m = *reinterpret_cast<const uint32_t *>(rp + SW_REC_FILL + wd * 4);
-            if (m == 0) continue;
-#pragma unroll 1
-            for (int g4 = 0; g4 < 8; ++g4) {
-                if (((m >> (4 * g4)) & 15u) == 0) continue;
-                const int sl = wd * 32 + g4 * 4 + (lane >> 3);
-                if ((m >> (4 * g4 + (lane >> 3))) & 1u)
-                    *reinterpret_cast<float4 *>(sg + (size_t)sl * SW_SLOT_BYTES + (lane & 7) * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+        // ---- zero fill: the record lists the slots of the [WY][WZ] grid that must be cleared (lattice point outside the
+        //      mesh and the buffer does not already hold zeros there): a warp takes 16 list entries, a quarter-warp 4 of
+        //      them (one 8-byte load), each slot cleared with 8 conflict-free 16-byte stores.  No search, no dependent
+        //      branches: walking a bitmap cost 800..3500 clocks per step, every word a dependent load behind the consumers' traffic.
+        {
+            const uint32_t e0 = (uint32_t)(pw * 16 + 4 * (lane >> 3));
+            if (e0 < nfill && nfill != HDR_NFILL_WHOLE) {
+                const uint2 four = *reinterpret_cast<const uint2 *>(rp + SW_REC_FLIST + 2 * e0);
+                unsigned char *const dst = sg + (lane & 7) * 16;
+                *reinterpret_cast<float4 *>(dst + (size_t)(four.x & 0xffffu) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (e0 + 1 < nfill) *reinterpret_cast<float4 *>(dst + (size_t)(four.x >> 16) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (e0 + 2 < nfill) *reinterpret_cast<float4 *>(dst + (size_t)(four.y & 0xffffu) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (e0 + 3 < nfill) *reinterpret_cast<float4 *>(dst + (size_t)(four.y >> 16) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
         // ---- V of the tile's own points (output planes only) and the store offsets of plane t - N ------------
@@ -357,19 +373,10 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
             else
                 mbar_arrive(bar);
         }
-        stage += G;
-        if (stage >= SW_STAGES) {   // G <= SW_STAGES: at most one wrap
-            stage -= SW_STAGES;
-            eparity ^= 1u;
-        }
-        rs += G;
-        if (rs >= SW_RING) {
-            rs -= SW_RING;
-            rparity ^= 1u;
-        }
         if (t + G < nsteps) {   // this group's next step: its record was requested SW_LOOKAHEAD steps before it
-            mbar_wait(rbar0 + 8u * rs, rparity);
-            fetch_v(rs);
+            const int rn = (t + G) % SW_RING;
+            mbar_wait(rbar0 + 8u * rn, (uint32_t)((t + G) / SW_RING) & 1u);
+            fetch_v(rn);
         }
     }
 }
@@ -577,9 +584,15 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     __shared__ uint64_t rec_bar[SW_RING];
     __shared__ uint32_t tmem_base_s;
 
-    // threads 0..PRODUCERS-1: the producer warps; then the consumer warps (the higher warp ids, which the warp
-    // scheduler favours when several warps are ready)
-    const int tid = threadIdx.x, ctid = tid - S::PRODUCERS, warp = tid >> 5;
+#ifndef SW_PROD_HIGH
+#define SW_PROD_HIGH 1
+#endif
+    // The warp scheduler favours the higher warp ids when several warps are ready.  The producers' instruction path is
+    // short but latency-critical (it paces every step), the consumers' is long and throughput-bound: the producer warps
+    // take the HIGH warp ids, so that they issue as soon as they can.
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const int ctid = SW_PROD_HIGH ? (tid < S::CONSUMERS ? tid : -1) : tid - S::PRODUCERS;
+    const int ptid = SW_PROD_HIGH ? tid - S::CONSUMERS : tid;
     const int2 item = a.items[blockIdx.x];
     const int nsteps = item.y;
     const long long clock0 = clock64();
@@ -594,7 +607,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
         for (int s = 0; s < SW_RING; ++s) mbar_init(smem_u32(&rec_bar[s]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    if (warp == S::PRODUCERS / 32) {   // first consumer warp
+    if (warp == (SW_PROD_HIGH ? 0 : S::PRODUCERS / 32)) {   // first consumer warp
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_base_s)),
                      "n"(SW_TMEM_COLS)
                      : "memory");
@@ -610,7 +623,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     if (ctid < 0) {
         setmaxnreg_dec<S::PROD_REGS>();
         sweep_producer<S, TENSOR>(a, maps, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), smem_u32(&rec_bar[0]),
-                                  a.recs + (size_t)item.x * S::REC_BYTES, nsteps, tid, 3.0 * w.w[0]);
+                                  a.recs + (size_t)item.x * S::REC_BYTES, nsteps, ptid, 3.0 * w.w[0]);
     } else {
         setmaxnreg_inc<S::CONS_REGS>();
         sweep_consumer<S>(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid,
@@ -849,6 +862,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                 // do not already hold zeros from an earlier plane staged in the same buffer
                 int nrun = 0;
                 uint32_t tx1 = 0, tx2 = 0;
+                uint32_t datamask[20] = {};   // slots that receive data from this plane's copy runs
                 for (int r = full ? 0 : N; r < (full ? WY : N + TY); ++r) {
                     const bool halo_row = r < N || r >= N + TY;
                     const int zlo = (halo_row || !full) ? N : 0, zhi = (halo_row || !full) ? N + TZ : WZ;
@@ -858,6 +872,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                         if (idx >= 0) {
                             if (run_start < 0) run_start = zp;
                             st[r * WZ + zp] = DATA;
+                            datamask[(r * WZ + zp) >> 5] |= 1u << ((r * WZ + zp) & 31);
                         } else {
                             if (run_start >= 0) {
                                 if (nrun >= SW_MAXRUN) return false;
@@ -878,7 +893,25 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                         }
                     }
                 }
-                hdrp[0] = g.warp_modes(pc.iy, pc.iz, p, full ? MODE_FULL : MODE_CENTRE) | (full ? HDR_OUTPUT_PLANE : 0u);
+                // the clear list: the set bits of the bitmap in ascending order; if there are more than the list holds, the
+                // kernel clears the WHOLE stage before the copies: then the bitmap names every slot without data
+                uint32_t nfill = 0;
+                uint16_t *flist = reinterpret_cast<uint16_t *>(rec + SW_REC_FLIST);
+                for (int sl = 0; sl < WY * WZ; ++sl) nfill += (fill[sl >> 5] >> (sl & 31)) & 1u;
+                if (nfill > (uint32_t)SW_MAXFILL) {
+                    for (int sl = 0; sl < WY * WZ; ++sl) {
+                        if (st[sl] == DATA && /* staged by THIS plane */ ((datamask[sl >> 5] >> (sl & 31)) & 1u)) continue;
+                        fill[sl >> 5] |= 1u << (sl & 31);
+                        st[sl] = ZERO;
+                    }
+                    nfill = HDR_NFILL_WHOLE;
+                } else {
+                    uint32_t q = 0;
+                    for (int sl = 0; sl < WY * WZ; ++sl)
+                        if ((fill[sl >> 5] >> (sl & 31)) & 1u) flist[q++] = (uint16_t)sl;
+                }
+                hdrp[0] = g.warp_modes(pc.iy, pc.iz, p, full ? MODE_FULL : MODE_CENTRE) | (full ? HDR_OUTPUT_PLANE : 0u) |
+                          (nfill << HDR_NFILL_SHIFT);
                 hdrp[1] = (uint32_t)(pc.chunk * SW_C);
                 hdrp[2] = tx1;
                 hdrp[3] = tx2;
@@ -1150,6 +1183,25 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
                 tx1 += len * SW_SLOT_BYTES;
             }
             if (tx1 != hdr[2]) return fail(cta, t, "byte count of the copy runs", 0, 0, 0);
+            {   // the clear list must name exactly the set bits of the bitmap; "whole stage": every slot without data is cleared
+                const uint32_t nf = (hdr[0] >> HDR_NFILL_SHIFT) & 0xffu;
+                const uint16_t *flist = reinterpret_cast<const uint16_t *>(rec + SW_REC_FLIST);
+                if (nf == HDR_NFILL_WHOLE) {
+                    std::vector<char> data((size_t)WY * WZ, 0);
+                    for (int r = 0; r < SW_MAXRUN; ++r)
+                        for (uint32_t i = 0; i < (runs[r].y >> 16); ++i) data[(runs[r].y & 0xffffu) + i] = 1;
+                    for (int sl = 0; sl < WY * WZ; ++sl)
+                        if ((((fill[sl >> 5] >> (sl & 31)) & 1u) != 0) == (data[sl] != 0)) return fail(cta, t, "whole-stage clear: bitmap", 0, 0, sl);
+                } else {
+                    uint32_t nbits = 0;
+                    for (int sl = 0; sl < WY * WZ; ++sl)
+                        if ((fill[sl >> 5] >> (sl & 31)) & 1u) {
+                            if (nbits >= nf || flist[nbits] != sl) return fail(cta, t, "clear list and bitmap differ", 0, 0, sl);
+                            ++nbits;
+                        }
+                    if (nbits != nf) return fail(cta, t, "clear list count", 0, 0, (int)nbits);
+                }
+            }
             for (int r = 0; r < WY; ++r)
                 for (int z = 0; z < WZ; ++z)
                     if ((fill[(r * WZ + z) >> 5] >> ((r * WZ + z) & 31)) & 1u) sg[r * WZ + z] = -1;

@@ -33,7 +33,7 @@ def _run(p, psi, n, B, kernel):
 
 # ---- config 0: tiny atom, nst=4, B=4 (BASELINE.json configs[0]) ---------------------------------
 @pytest.mark.parametrize("kernel", ["auto", "gather", "sweep"])
-@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX])
+@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX, rs.RS_ORDER_TILE])
 def test_config0(kernel, ordering):
     p = problem(0, ordering)
     cfg = p.cfg

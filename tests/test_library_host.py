@@ -42,7 +42,7 @@ def _sets_equal(lib_ijk, omesh):
     return a == b, (a - b, b - a)
 
 
-@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX])
+@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX, rs.RS_ORDER_TILE])
 @pytest.mark.parametrize("cfg_i", [0, 1])
 def test_mesh_point_set_equals_oracle(cfg_i, ordering):
     cfg = synthetic.config(cfg_i)
@@ -93,7 +93,7 @@ def _bruteforce_map(ijk, n, periodic_box=None):
     return out
 
 
-@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX])
+@pytest.mark.parametrize("ordering", [rs.RS_ORDER_BRICK, rs.RS_ORDER_LEX, rs.RS_ORDER_TILE])
 @pytest.mark.parametrize("n", [1, 4, 6])
 def test_index_map_matches_definition_and_invariants(n, ordering):
     cfg = synthetic.config(0)
