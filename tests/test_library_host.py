@@ -56,6 +56,14 @@ def test_mesh_point_set_equals_oracle(cfg_i, ordering):
     if ordering == rs.RS_ORDER_LEX:
         assert np.array_equal(ijk, om.ijk())
         assert np.array_equal(synthetic.canonical_rank(ijk), np.arange(m.npoints))
+    elif ordering == rs.RS_ORDER_TILE:
+        # i decreases only where the enumeration moves on to the next tile column (the tile origin is the library's)
+        ext = ijk.max(axis=0) - ijk.min(axis=0) + 1
+        ncols = (ext[1] // 16 + 2) * (ext[2] // 16 + 2)
+        assert (np.diff(ijk[:, 0]) < 0).sum() < ncols and m.nbricks == 0
+        same_plane = np.diff(ijk[:, 0]) == 0                   # inside a tile plane: (j, k) ascending, within 16 x 16
+        dj, dk = np.diff(ijk[:, 1])[same_plane], np.diff(ijk[:, 2])[same_plane]
+        assert ((dj > 0) | ((dj == 0) & (dk > 0))).all() and np.abs(dj).max() < 16 and np.abs(dk).max() < 16
     else:
         assert m.nbricks > 0
     # canonical_rank agrees with the oracle's own ranking of the same points
