@@ -1296,6 +1296,18 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
     if (!rs_sweep_supported(m, n, ncol)) return RS_OK;   // the gather kernel serves this call: nothing to tune
     const auto key = std::make_pair(n * 16 + sweep_variant(n), ncol);
     rs_sweep_costs costs;
+    // The measured costs depend a little on what runs beside a step, so a re-deal is not always better than the one before:
+    // every dealing's slowest CTA is measured, and the best dealing seen (possibly the modelled one) is the one kept.
+    long long best_max = -1;
+    bool best_is_model = true, cur_is_model = m->sweep_costs.find(key) == m->sweep_costs.end();
+    rs_sweep_costs best_costs, cur_costs;
+    if (!cur_is_model) cur_costs = m->sweep_costs[key];
+    auto slowest_cta = [&](const rs_sweep_tables *tb, long long *out) -> rs_status {
+        std::vector<long long> cyc((size_t)tb->nitems);
+        RS_CUDA_TRY(cudaMemcpy(cyc.data(), tb->d_cycles, cyc.size() * sizeof(long long), cudaMemcpyDeviceToHost));
+        *out = *std::max_element(cyc.begin(), cyc.end());
+        return RS_OK;
+    };
     for (int round = 0; round < (m->opt.tune_rounds < 1 ? 1 : m->opt.tune_rounds); ++round) {   // later rounds measure the re-dealt work and refine it
         const rs_sweep_tables *tb = nullptr;
         rs_status rc = get_tables(m, n, ncol, &tb);
@@ -1306,6 +1318,12 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
             if (rc != RS_OK) return rc;
         }
         RS_CUDA_TRY(cudaStreamSynchronize(st));
+        {
+            long long mx = 0;
+            rc = slowest_cta(tb, &mx);
+            if (rc != RS_OK) return rc;
+            if (best_max < 0 || mx < best_max) best_max = mx, best_is_model = cur_is_model, best_costs = cur_costs;
+        }
         std::vector<long long> clk((size_t)tb->nrec + 1);
         RS_CUDA_TRY(cudaMemcpy(clk.data(), tb->d_step_clock, clk.size() * sizeof(long long), cudaMemcpyDeviceToHost));
         size_t ncell = 0;
@@ -1335,6 +1353,7 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
         costs.halo = halo_sum / halo_n;
         costs.unit = full_sum / full_n;
         m->sweep_costs[key] = costs;
+        cur_costs = costs, cur_is_model = false;
         // drop the tables: the next use builds them with the measured costs
         auto f = m->sweep.find(key);
         if (f != m->sweep.end()) {
@@ -1343,9 +1362,33 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
             m->sweep.erase(f);
         }
     }
-    // one measuring launch on the final tables: rs_sweep_stats then describes the dealing now in use
-    rs_status rc = launch_sweep(m, n, w, vloc, psi, hpsi, ncol, st, true);
-    if (rc != RS_OK) return rc;
-    RS_CUDA_TRY(cudaStreamSynchronize(st));
+    // one measuring launch on the final tables (rs_sweep_stats then describes the dealing in use); if an earlier dealing
+    // was faster, go back to it
+    auto drop_tables = [&]() {
+        auto f = m->sweep.find(key);
+        if (f != m->sweep.end()) {
+            rs_sweep_tables &t = f->second;
+            cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles), cudaFree(t.d_step_clock);
+            m->sweep.erase(f);
+        }
+    };
+    for (int pass = 0; pass < 2; ++pass) {
+        rs_status rc = launch_sweep(m, n, w, vloc, psi, hpsi, ncol, st, true);
+        if (rc != RS_OK) return rc;
+        RS_CUDA_TRY(cudaStreamSynchronize(st));
+        if (pass == 1) break;
+        const rs_sweep_tables *tb = nullptr;
+        rc = get_tables(m, n, ncol, &tb);
+        if (rc != RS_OK) return rc;
+        long long mx = 0;
+        rc = slowest_cta(tb, &mx);
+        if (rc != RS_OK) return rc;
+        if (best_max < 0 || mx <= best_max) break;     // the last dealing is the best one
+        if (best_is_model)
+            m->sweep_costs.erase(key);
+        else
+            m->sweep_costs[key] = best_costs;
+        drop_tables();
+    }
     return RS_OK;
 }

@@ -99,12 +99,13 @@ def test_block_axpy_and_copy(B, nst, is_complex):
     assert torch.all(Y[p.np] == 0)                                  # the zero slot stays zero
 
 
-@pytest.mark.parametrize("B,is_complex", [(4, False), (16, False), (32, False), (8, True)])
-def test_apply_ex_sums_match_the_oracle(B, is_complex):
-    """H psi and the per-orbital sums of one eigensolver step from ONE call, config 1 (gather and plane-sweep kernels)."""
+@pytest.mark.parametrize("cfg_i,B,is_complex", [(1, 4, False), (1, 16, False), (1, 32, False), (1, 8, True), (2, 16, False)])
+def test_apply_ex_sums_match_the_oracle(cfg_i, B, is_complex):
+    """H psi and the per-orbital sums of one eigensolver step from ONE call (config 1; config 2 at full size): gather kernel
+    (B = 4) or plane-sweep kernel (B >= 16 real columns) followed by the streaming reduction kernel."""
     import torch
 
-    p = problem(1)
+    p = problem(cfg_i)
     n = 4
     psi = synthetic.orbitals(77, 0, B, p.np, is_complex=is_complex)
     blk = to_block(p, psi, B)
