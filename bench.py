@@ -212,6 +212,9 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-autotune", action="store_true", help="skip rs_hamiltonian_autotune (work dealt by the built-in cost model)")
+    ap.add_argument("--ordering", default="lex", choices=["lex", "brick", "tile"],
+                    help="point enumeration of the mesh (ordering study; brick / tile are served by the gather kernel)")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the timings of the f1-f3 operations (SURVEY.md 8(f))")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
@@ -247,7 +250,8 @@ def main() -> None:
 
     # ---- once per geometry: mesh tables (a1-a3), potential, inputs --------------------------------
     t = time.perf_counter()
-    mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, max(cfg.fd_orders))
+    ordering = {"lex": rs.RS_ORDER_LEX, "brick": rs.RS_ORDER_BRICK, "tile": rs.RS_ORDER_TILE}[args.ordering]
+    mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, max(cfg.fd_orders), ordering)
     t_mesh = time.perf_counter() - t
     npts = mesh.npoints
     ijk = mesh.points()
@@ -256,8 +260,8 @@ def main() -> None:
     # weak scaling: every rank owns its own nst orbitals (orbital ids rank*nst ...), same mesh and V
     host_states = torch.empty((nst, npts), dtype=tdt).pin_memory()
     hs = host_states.numpy()
-    for j in range(nst):
-        hs[j] = synthetic.orbital(cfg.seed, rank * nst + j, npts, is_c)[rank_of]
+    for j, ist in enumerate(synthetic.rank_orbital_ids(rank, nst)):
+        hs[j] = synthetic.orbital(cfg.seed, ist, npts, is_c)[rank_of]
     host_out = torch.empty((nst, npts), dtype=tdt).pin_memory()
     host_v = torch.from_numpy(v_mesh).pin_memory()
 
@@ -391,6 +395,55 @@ def main() -> None:
                           "note": "block working set may fit L2" if 2 * b1.numel() * b1.element_size() < 126e6 else ""})
             del b1, b2
 
+    # ---- the operations around H psi on the same block: time and algorithmic rates -------
+    next_rows = None
+    if not args.no_next_rows and rank == 0:
+        def timed(fn, reps=20):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(reps):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / reps
+        rs.rs_block_pack(mesh, states, 0, min(B, nst), B, blk)
+        rs.rs_hamiltonian_apply(mesh, n, coeffs, v, blk, hblk, B, kernel=kern)
+        blk_bytes = npts * B * 8 * lanes
+        sums = torch.empty((3, B), dtype=torch.float64, device=dev)
+        eps_d = torch.zeros(B, dtype=torch.float64, device=dev)
+        Mm = torch.empty((B, B), dtype=tdt, device=dev)
+        alpha = torch.ones(B, dtype=tdt, device=dev)
+        ms_exp = timed(lambda: rs.rs_block_expectation(mesh, blk, hblk, eps_d, B, sums))
+        ms_ex = timed(lambda: rs.rs_hamiltonian_apply_ex(mesh, n, coeffs, v, blk, hblk, B, eps_d, sums))
+        ms_ovl = timed(lambda: rs.rs_block_overlap(mesh, blk, hblk, B, Mm))
+        ms_axpy = timed(lambda: rs.rs_block_axpy(mesh, alpha, blk, hblk, B))
+        rs.rs_hamiltonian_apply(mesh, n, coeffs, v, blk, hblk, B, kernel=kern)
+        rc_nl, lmax = 2.0, 1
+        nl = rs.rs_nonlocal_create(mesh, cfg.centers, rc_nl, (lmax + 1) ** 2)
+        nsph = 0
+        for A in range(cfg.centers.shape[0]):
+            idx = nl.sphere(A)
+            nsph += idx.size
+            nl.set_projectors(A, synthetic.projector_values(ijk[idx].astype(np.float64) * cfg.spacing - cfg.centers[A], lmax, 0.7))
+        nl.prepare()
+        ms_nl = timed(lambda: rs.rs_nonlocal_apply(nl, blk, hblk, B))
+        nlm = (lmax + 1) ** 2
+        next_rows = {
+            "f1_expectation": {"ms": ms_exp, "alg_gbs": 2 * blk_bytes / ms_exp / 1e6, "frac_measured": 2 * blk_bytes / ms_exp / 1e6 / peak},
+            "f1_apply_ex": {"ms": ms_ex, "extra_over_apply": ms_ex / apply_ms - 1.0,
+                            "note": "apply + streaming reduction kernel (a fused consumer epilogue was measured slower, DESIGN.md)"},
+            "f1_axpy": {"ms": ms_axpy, "alg_gbs": 3 * blk_bytes / ms_axpy / 1e6, "frac_measured": 3 * blk_bytes / ms_axpy / 1e6 / peak},
+            "f2_overlap": {"ms": ms_ovl, "alg_gbs": 2 * blk_bytes / ms_ovl / 1e6, "frac_measured": 2 * blk_bytes / ms_ovl / 1e6 / peak,
+                           "tflops_executed": 2.0 * npts * (B * lanes) ** 2 / ms_ovl / 1e9, "kernel": "overlap_kernel (fp64 DMMA m8n8k4)"},
+            "f3_nonlocal": {"ms": ms_nl, "atoms": int(cfg.centers.shape[0]), "rc": rc_nl, "nlm": nlm, "sphere_points": int(nsph),
+                            "colors": nl.ncolors, "gflops_executed": 4.0 * nsph * B * lanes * nlm / ms_nl / 1e6,
+                            "alg_gbs": nsph * (3 * B * lanes * 8 + 2 * nlm * 8 + 4) / ms_nl / 1e6},
+        }
+        del nl
+
     # ---- end to end through the host-buffer entry point (a7 workspace, created once) ---------------
     e2e = None
     if not args.no_e2e:
@@ -435,13 +488,15 @@ def main() -> None:
                 "vs_baseline": None, "dtype": "c128" if is_c else "f64", "data": "synthetic",
                 "config": {**workload_config(cfg, n, B, npts, nst), "kernel": kname, "parallelism": f"orbital-blocks x{world}",
                            "mesh_build_s": t_mesh, "prepare_s": t_prepare, "autotune_s": t_tune, "autotuned": tune,
-                           "nbricks": mesh.nbricks},
+                           "nbricks": mesh.nbricks, "ordering": args.ordering},
                 "value_executed_flops": world * nst * npts * flops_per_output(n) * lanes / (ms_step * 1e-3) / 1e9,
                 "flop_convention": "BASELINE.json: nst*np*(2*(6n+1)+2), x4 for complex; *_executed counts the arithmetic "
                                    "actually done (complex = 2 real lanes, reading S12)",
                 "roofline": roofline, "clocks": clocks, "gpu_launches": 3 * nblocks * args.steps}
         if blocked:
             line["blocked_resident"] = blocked
+        if next_rows:
+            line["next_rows"] = next_rows
         if e2e:
             line["e2e"] = e2e
         if sweep:

@@ -160,6 +160,12 @@ def shard_orbitals(nst_total: int, block: int, rank: int, world: int) -> tuple[i
     return min(lo * block, nst_total), min(hi * block, nst_total)
 
 
+def rank_orbital_ids(rank: int, nst: int) -> range:
+    """Weak scaling of bench.py (--gpus N): every rank owns its own nst orbitals of the same mesh, ids rank*nst ..
+    (rank+1)*nst - 1; no rank ever needs another rank's orbitals (orbitals are independent)."""
+    return range(rank * nst, (rank + 1) * nst)
+
+
 def canonical_rank(ijk: np.ndarray) -> np.ndarray:
     """rank[ip] = position of mesh point ip in the canonical (lexicographic i, j, k) order of the same
     point set.  `ijk` is whatever enumeration a mesh builder publishes; orbitals generated in

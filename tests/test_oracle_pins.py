@@ -295,12 +295,15 @@ def test_P9_union_is_union_of_single_spheres():
 def test_P10_fig4_layout():
     """4 orbitals x 5 coefficients: element (orbital j, coefficient p) sits at j*5+p in the standard
     layout and at p*4+j in the blocked layout."""
-    states = np.arange(20, dtype=np.float64).reshape(4, 5)       # value = standard-layout address
-    blk = oracle.block_pack(states, 0, 4, 4, 5, 5)
+    dims = dict(line.split() for line in open(os.path.join(GOLD, "fig4_layout.txt")) if not line.startswith("#"))
+    norb, ncoef = int(dims["norbitals"]), int(dims["ncoeff"])
+    assert (norb, ncoef) == (4, 5)                                # the figure's own sizes
+    states = np.arange(norb * ncoef, dtype=np.float64).reshape(norb, ncoef)   # value = standard-layout address
+    blk = oracle.block_pack(states, 0, norb, norb, ncoef, ncoef)
     flat = blk.ravel()
-    for j in range(4):
-        for p in range(5):
-            assert flat[p * 4 + j] == j * 5 + p
+    for j in range(norb):
+        for p in range(ncoef):
+            assert flat[p * norb + j] == j * ncoef + p
     # the arrows of Fig. 4: first coefficient of orbital j moves from address 5j to address j
     assert [int(flat[j]) for j in range(4)] == [0, 5, 10, 15]
 

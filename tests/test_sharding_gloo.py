@@ -2,7 +2,9 @@
 (orbitals are independent).  Each rank takes the contiguous range of
 whole blocks that synthetic.shard_orbitals deals it, computes H psi for that range with the oracle standing in
 for the device (no GPU here), and the gathered result must equal the unsharded one; the max-over-ranks timing
-reduction bench.py uses is exercised too."""
+reduction bench.py uses is exercised too.  What runs of the product here: every rank builds its own replica of the
+mesh through librs.so (host tables only: mesh, plane-sweep records and their replay) and the replicas must be
+identical; the kernels themselves need a device.  No multi-GPU run exists (gpurun gives one GPU)."""
 import os
 import socket
 
@@ -40,6 +42,18 @@ def _worker(rank, world, port, nst, block, out_path):
     dist.all_reduce(ms, op=dist.ReduceOp.MAX)            # bench.py's max-over-ranks timing
     ranges = [None] * world
     dist.all_gather_object(ranges, (lo, hi))
+    # the product's replicated set-up: each rank builds the mesh and the sweep records itself
+    import hashlib
+    import paper_1306_2953_b200 as rs
+    mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, 4)
+    st = rs.rs_sweep_selfcheck(mesh, 4, 16)
+    digest = hashlib.sha256(mesh.points().tobytes()).hexdigest() + f":{st['records']}:{st['table_bytes']}"
+    digests = [None] * world
+    dist.all_gather_object(digests, digest)
+    assert len(set(digests)) == 1 and mesh.npoints == om.npoints
+    ids = [None] * world
+    dist.all_gather_object(ids, list(synthetic.rank_orbital_ids(rank, nst)))
+    assert sorted(sum(ids, [])) == list(range(world * nst))          # bench.py's weak-scaling ownership: disjoint, complete
     if rank == 0:
         np.savez(out_path, h=t.numpy(), ms=ms.numpy(), ranges=np.array(ranges))
     dist.barrier()
