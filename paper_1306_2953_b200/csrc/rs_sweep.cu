@@ -65,15 +65,15 @@ constexpr int SW_NBOX = 6;               // tensor-map box heights 1, 2, 4, 8, 1
 // NGROUPS producer groups of 4 warps.  Compiled shapes (rs_sweep_variant()):
 //   <4, 16, 4, 2>  fd_order 4: 8 consumer warps, 16 outputs per thread, 4 pending planes in registers
 //   <6,  8, 2, 2>  fd_order 6: 6 pending planes of a 4 x 4 patch do not fit the register file; 2 x 4 patches do
-template <int N_, int TY_, int PY_, int NGROUPS_>
+template <int N_, int TY_, int PY_, int NGROUPS_, int GW_ = 4>
 struct sweep_shape {
-    static constexpr int N = N_, TY = TY_, PY = PY_, NGROUPS = NGROUPS_;
+    static constexpr int N = N_, TY = TY_, PY = PY_, NGROUPS = NGROUPS_, GW = GW_;   // GW: warps per producer group
     static constexpr int WY = TY + 2 * N, WZ = SW_TZ + 2 * N;            // rows / z-slots of a staged plane
     static constexpr int STAGE_BYTES = WY * WZ * SW_SLOT_BYTES;         // uniform [WY][WZ] slots; the corners hold V, offsets, header
     static constexpr int NPT = TY * SW_TZ;                              // tile points
     static constexpr int CONSUMERS = (TY / PY) * (SW_TZ / SW_PZ) * SW_C;   // one thread per (patch, column)
     static constexpr int NCW = CONSUMERS / 32;
-    static constexpr int PRODUCERS = 128 * NGROUPS;
+    static constexpr int PRODUCERS = 32 * GW * NGROUPS;
     static constexpr int THREADS = PRODUCERS + CONSUMERS;
     static constexpr int REC_BYTES = SW_REC_CIDX + NPT * 4;
     static constexpr int ROW_WORDS = N * 2 * SW_PZ;                      // tensor memory: one patch row = N ring slots x 4 doubles
@@ -84,14 +84,16 @@ struct sweep_shape {
     static constexpr int LAUNCH_REGS = (65536 / THREADS) & ~7;
     static constexpr int PROD_REGS = 32;
     static constexpr int CONS_REGS = (LAUNCH_REGS + (LAUNCH_REGS - PROD_REGS) * PRODUCERS / CONSUMERS) & ~7;
-    static_assert(TY % PY == 0 && 4 % PY == 0 && CONSUMERS % 128 == 0 && N % NGROUPS == 0, "shape");
+    static_assert(TY % PY == 0 && 4 % PY == 0 && CONSUMERS % 128 == 0 && N % NGROUPS == 0 && (GW == 4 || GW == 8), "shape");
     static_assert(TY <= 4 * N && N >= 4, "the corners must hold V (512 bytes per corner row) and the offsets");
     static_assert(REC_BYTES % 16 == 0 && SMEM + 256 <= 232448, "shared memory budget");
     static_assert((NCW + 3) / 4 * PY * ROW_WORDS <= SW_TMEM_COLS, "tensor memory budget");
     static_assert(WY * WZ <= 18 * 32, "zero-fill bitmap");
 };
-using shape_n4 = sweep_shape<4, 16, 4, 2>;
-using shape_n6 = sweep_shape<6, 8, 2, 2>;
+// two groups of 4 producer warps alternate steps (one group of 8 warps staging every step was measured 4 % slower:
+// 0.127 against 0.122 ms on config 2, B = 16)
+using shape_n4 = sweep_shape<4, 16, 4, 2, 4>;
+using shape_n6 = sweep_shape<6, 8, 2, 2, 4>;
 
 // the same numbers at run time, for the host-side builder
 struct shape_rt {
@@ -247,10 +249,11 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
                                                uint32_t full0, uint32_t empty0, uint32_t rbar0, const unsigned char *recs,
                                                int nsteps, int ptid, double w0x3)
 {
-    constexpr int N = S::N, G = S::NGROUPS;
-    constexpr int PPT = (S::NPT + 127) / 128;   // tile points per thread (V and offsets)
-    constexpr int HS = N / G;                   // a plane's store offsets are staged HS own steps after the plane itself
-    const int group = ptid >> 7, gtid = ptid & 127, lane = ptid & 31, pw = gtid >> 5;
+    constexpr int N = S::N, G = S::NGROUPS, GW = S::GW, GT = 32 * GW;   // GT threads per group
+    constexpr int PPT = (S::NPT + GT - 1) / GT;   // tile points per thread (V and offsets)
+    constexpr int HS = N / G;                     // a plane's store offsets are staged HS own steps after the plane itself
+    constexpr int D = G == 1 ? 2 : 1;             // V and the offsets are fetched D own steps ahead (>= one full step period)
+    const int group = ptid / GT, gtid = ptid % GT, lane = ptid & 31, pw = gtid >> 5;
     unsigned char *const ring = smem + (size_t)SW_STAGES * S::STAGE_BYTES;
     const uint32_t sbase = smem_u32(smem);
     auto request_rec = [&](int r) {   // one thread; preceded by a fence.proxy.async of that thread
@@ -261,11 +264,11 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
     if (ptid == 0)
         for (int r = 0; r < SW_LOOKAHEAD && r < nsteps; ++r) request_rec(r);
     // this thread's jobs: copy run `myrun` (lanes 0..15 of each warp), a share of the zero fill, tile points gtid (+ 128)
-    const int myrun = lane * 4 + pw;
+    const int myrun = lane * GW + pw;
     // point p = (ty, tz): V at corner A row ty / 4, offsets at corner B row ty / 4 (4 tile rows per corner row)
     const uint32_t v_off0 = (uint32_t)(((gtid >> 6) * S::WZ) * SW_SLOT_BYTES + (gtid & 63) * 8);
     const uint32_t i_off0 = (uint32_t)(((gtid >> 6) * S::WZ + S::WZ - N) * SW_SLOT_BYTES + (gtid & 63) * 4);
-    constexpr uint32_t NEXT_POINT = 2 * S::WZ * SW_SLOT_BYTES;   // point gtid + 128: two corner rows further
+    constexpr uint32_t NEXT_POINT = (GT / 64) * S::WZ * SW_SLOT_BYTES;   // point gtid + GT: GT / 64 corner rows further
     // stage = t mod SW_STAGES, record slot rs = t mod SW_RING and the barrier parities are re-derived from t where they are
     // needed instead of being carried: the producers run on 32 registers and a spilled V value would put the global-load
     // latency back on the per-step path (the first pass over the stages finds them free: parity 1)
@@ -274,28 +277,43 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
     // ~1000 clocks per step: measured 0.136 -> 0.127 ms on config 2).  The store offsets of a plane's outputs are needed N steps later, when the x arm is
     // complete: this group staged that plane too (N is a multiple of the number of groups), so each thread simply
     // remembers its points' offsets for HS of its own steps and stages them with plane t.
-    double vv[PPT];
-    uint32_t of[PPT], hist[HS][PPT];
+    double vv[D][PPT];             // vv[0]: this own step's V, vv[D-1]: the value fetched last
+    uint32_t hist[HS + D][PPT];    // offsets by age in own steps: hist[D-1] fetched last, hist[0] this step's, hist[HS] staged now
 #pragma unroll
     for (int q = 0; q < PPT; ++q) {
-        vv[q] = 0.0, of[q] = 0xffffffffu;
 #pragma unroll
-        for (int h = 0; h < HS; ++h) hist[h][q] = 0xffffffffu;
+        for (int d = 0; d < D; ++d) vv[d][q] = 0.0;
+#pragma unroll
+        for (int h = 0; h < HS + D; ++h) hist[h][q] = 0xffffffffu;
     }
-    auto fetch_v = [&](int slot) {
+    // shift the queues by one own step and fetch the V / offsets of the own step D - 1 ahead of the next one (record slot `slot`)
+    auto advance_and_fetch = [&](int slot, bool have) {
+#pragma unroll
+        for (int q = 0; q < PPT; ++q) {
+#pragma unroll
+            for (int h = HS + D - 1; h > 0; --h) hist[h][q] = hist[h - 1][q];
+#pragma unroll
+            for (int d = 0; d + 1 < D; ++d) vv[d][q] = vv[d + 1][q];
+            hist[0][q] = 0xffffffffu;
+            vv[D - 1][q] = 0.0;
+        }
+        if (!have) return;
         const unsigned char *rp = ring + (size_t)slot * S::REC_BYTES;
         const uint32_t coff = *reinterpret_cast<const uint32_t *>(rp + SW_REC_HDR + 4);
 #pragma unroll
         for (int q = 0; q < PPT; ++q) {
-            const int p = gtid + 128 * q;
+            const int p = gtid + GT * q;
             const int32_t ci = p < S::NPT ? *reinterpret_cast<const int32_t *>(rp + SW_REC_CIDX + p * 4) : -1;
-            vv[q] = ci >= 0 ? __ldg(a.vloc + ci) : -w0x3;   // consumed one own step later, when 3 w_0 is added: no wait here
-            of[q] = ci >= 0 ? (uint32_t)ci * a.ncol + coff : 0xffffffffu;
+            vv[D - 1][q] = ci >= 0 ? __ldg(a.vloc + ci) : -w0x3;   // consumed D own steps later, when 3 w_0 is added: no wait here
+            hist[0][q] = ci >= 0 ? (uint32_t)ci * a.ncol + coff : 0xffffffffu;
         }
     };
-    if (group < nsteps) {
-        mbar_wait(rbar0 + 8u * group, 0u);
-        fetch_v(group);
+    // prologue: the first D own steps' values (own step k of this group is step group + k * G)
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+        const int tt = group + d * G;
+        if (tt < nsteps) mbar_wait(rbar0 + 8u * (tt % SW_RING), (uint32_t)(tt / SW_RING) & 1u);
+        advance_and_fetch(tt % SW_RING, tt < nsteps);
     }
     for (int t = group; t < nsteps; t += G) {
         const int stage = t % SW_STAGES, rs = t % SW_RING;
@@ -308,7 +326,7 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         const uint32_t bar = full0 + 8u * stage;
         const uint4 hdr = *reinterpret_cast<const uint4 *>(rp + SW_REC_HDR);   // {modes|flags, column offset, tx bytes 1-D, tx bytes 2-D}
         uint2 run = make_uint2(0u, 0u);
-        if (lane < SW_MAXRUN / 4) run = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
+        if (lane < SW_MAXRUN / GW) run = *reinterpret_cast<const uint2 *>(rp + SW_REC_RUNS + myrun * 8);
         const uint32_t len = run.y >> 16, slot = run.y & 0xffffu;
         mbar_wait(empty0 + 8u * stage, eparity);
         const uint32_t nfill = (hdr.x >> HDR_NFILL_SHIFT) & 0xffu;
@@ -316,9 +334,9 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
             // a piece's first planes: more slots to clear than the list holds -> the group clears the whole stage, and only
             // then (group barrier) may any of its warps issue the plane's copies
 #pragma unroll 1
-            for (uint32_t o = (uint32_t)gtid * 16u; o < (uint32_t)S::STAGE_BYTES; o += 128u * 16u)
+            for (uint32_t o = (uint32_t)gtid * 16u; o < (uint32_t)S::STAGE_BYTES; o += (uint32_t)GT * 16u)
                 *reinterpret_cast<float4 *>(sg + o) = make_float4(0.f, 0.f, 0.f, 0.f);
-            named_bar_sync(2 + group, 128);
+            named_bar_sync(2 + group, GT);
         }
         fence_proxy_async();   // earlier generic accesses to this stage and to the record slot reused below (ordered before us by the barrier) before our async copies
         // ---- copy runs --------------------------------------------------------------------------------
@@ -340,28 +358,31 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
         //      them (one 8-byte load), each slot cleared with 8 conflict-free 16-byte stores.  No search, no dependent
         //      branches: walking a bitmap cost 800..3500 clocks per step, every word a dependent load behind the consumers' traffic.
         {
-            const uint32_t e0 = (uint32_t)(pw * 16 + 4 * (lane >> 3));
+            constexpr int EPQ = SW_MAXFILL / GW / 4;   // list entries per quarter-warp: 4 (one 8-byte load) or 2 (one 4-byte load)
+            const uint32_t e0 = (uint32_t)(pw * (SW_MAXFILL / GW) + EPQ * (lane >> 3));
             if (e0 < nfill && nfill != HDR_NFILL_WHOLE) {
-                const uint2 four = *reinterpret_cast<const uint2 *>(rp + SW_REC_FLIST + 2 * e0);
+                uint32_t ent[2];
+                if constexpr (EPQ == 4) {
+                    const uint2 four = *reinterpret_cast<const uint2 *>(rp + SW_REC_FLIST + 2 * e0);
+                    ent[0] = four.x, ent[1] = four.y;
+                } else {
+                    ent[0] = *reinterpret_cast<const uint32_t *>(rp + SW_REC_FLIST + 2 * e0), ent[1] = 0;
+                }
                 unsigned char *const dst = sg + (lane & 7) * 16;
-                *reinterpret_cast<float4 *>(dst + (size_t)(four.x & 0xffffu) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (e0 + 1 < nfill) *reinterpret_cast<float4 *>(dst + (size_t)(four.x >> 16) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (e0 + 2 < nfill) *reinterpret_cast<float4 *>(dst + (size_t)(four.y & 0xffffu) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (e0 + 3 < nfill) *reinterpret_cast<float4 *>(dst + (size_t)(four.y >> 16) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int i = 0; i < EPQ; ++i)
+                    if (e0 + i < nfill)
+                        *reinterpret_cast<float4 *>(dst + (size_t)((ent[i >> 1] >> (16 * (i & 1))) & 0xffffu) * SW_SLOT_BYTES) = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
         // ---- V of the tile's own points (output planes only) and the store offsets of plane t - N ------------
 #pragma unroll
         for (int q = 0; q < PPT; ++q) {
-            if (gtid + 128 * q < S::NPT) {
+            if (gtid + GT * q < S::NPT) {
                 if (hdr.x & HDR_OUTPUT_PLANE)   // 3 w_0 + V: the whole diagonal coefficient
-                    *reinterpret_cast<double *>(sg + v_off0 + q * NEXT_POINT) = vv[q] + w0x3;
-                *reinterpret_cast<uint32_t *>(sg + i_off0 + q * NEXT_POINT) = hist[HS - 1][q];
+                    *reinterpret_cast<double *>(sg + v_off0 + q * NEXT_POINT) = vv[0][q] + w0x3;
+                *reinterpret_cast<uint32_t *>(sg + i_off0 + q * NEXT_POINT) = hist[HS + D - 1][q];
             }
-#pragma unroll
-            for (int h = HS - 1; h > 0; --h) hist[h][q] = hist[h - 1][q];
-            hist[0][q] = of[q];
-            of[q] = 0xffffffffu;
         }
         if (gtid == 0) *reinterpret_cast<uint2 *>(sg + S::HDR_OFF) = make_uint2(hdr.x, hdr.y);
         __syncwarp();
@@ -373,10 +394,10 @@ __device__ __forceinline__ void sweep_producer(const sweep_args &a, const sweep_
             else
                 mbar_arrive(bar);
         }
-        if (t + G < nsteps) {   // this group's next step: its record was requested SW_LOOKAHEAD steps before it
-            const int rn = (t + G) % SW_RING;
-            mbar_wait(rbar0 + 8u * rn, (uint32_t)((t + G) / SW_RING) & 1u);
-            fetch_v(rn);
+        {   // the queues move on by one own step; fetch for the own step D ahead (its record was requested SW_LOOKAHEAD steps before it)
+            const int tn = t + D * G;
+            if (tn < nsteps) mbar_wait(rbar0 + 8u * (tn % SW_RING), (uint32_t)(tn / SW_RING) & 1u);
+            advance_and_fetch(tn % SW_RING, tn < nsteps);
         }
     }
 }
@@ -600,7 +621,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < SW_STAGES; ++s) {
-            mbar_init(smem_u32(&full_bar[s]), 4);   // the 4 warps of the producer group that stages the step
+            mbar_init(smem_u32(&full_bar[s]), S::GW);   // the warps of the producer group that stages the step
             mbar_init(smem_u32(&empty_bar[s]), S::NCW);
         }
 #pragma unroll
