@@ -214,6 +214,8 @@ def main() -> None:
     ap.add_argument("--no-autotune", action="store_true", help="skip rs_hamiltonian_autotune (work dealt by the built-in cost model)")
     ap.add_argument("--ordering", default="lex", choices=["lex", "brick", "tile"],
                     help="point enumeration of the mesh (ordering study; brick / tile are served by the gather kernel)")
+    ap.add_argument("--planes-tuned", type=int, default=0,
+                    help="x-slab thickness of the plane-sweep work pieces after autotune (0: library default = whole tile columns)")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the timings of the f1-f3 operations (SURVEY.md 8(f))")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -253,6 +255,8 @@ def main() -> None:
     ordering = {"lex": rs.RS_ORDER_LEX, "brick": rs.RS_ORDER_BRICK, "tile": rs.RS_ORDER_TILE}[args.ordering]
     mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, max(cfg.fd_orders), ordering)
     t_mesh = time.perf_counter() - t
+    if args.planes_tuned:
+        rs.rs_mesh_set_sweep_options(mesh, planes_tuned=args.planes_tuned)
     npts = mesh.npoints
     ijk = mesh.points()
     v_mesh = synthetic.vloc_at(ijk.astype(np.float64) * cfg.spacing, cfg.centers, cfg.charges)
@@ -488,7 +492,7 @@ def main() -> None:
                 "vs_baseline": None, "dtype": "c128" if is_c else "f64", "data": "synthetic",
                 "config": {**workload_config(cfg, n, B, npts, nst), "kernel": kname, "parallelism": f"orbital-blocks x{world}",
                            "mesh_build_s": t_mesh, "prepare_s": t_prepare, "autotune_s": t_tune, "autotuned": tune,
-                           "nbricks": mesh.nbricks, "ordering": args.ordering},
+                           "nbricks": mesh.nbricks, "ordering": args.ordering, "planes_tuned": args.planes_tuned or "whole columns"},
                 "value_executed_flops": world * nst * npts * flops_per_output(n) * lanes / (ms_step * 1e-3) / 1e9,
                 "flop_convention": "BASELINE.json: nst*np*(2*(6n+1)+2), x4 for complex; *_executed counts the arithmetic "
                                    "actually done (complex = 2 real lanes, reading S12)",
