@@ -89,9 +89,9 @@ static rs_status check_blocks(const rs_mesh *m, const void *a, const void *b, in
 
 extern "C" rs_status rs_block_dot(const rs_mesh *m, const void *a, const void *b, int nst, rs_dtype dtype, void *out_dev, void *stream)
 {
+    if (!out_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_dot: null output");
     rs_status st = check_blocks(m, a, b, nst, dtype, "rs_block_dot");
     if (st != RS_OK) return st;
-    if (!out_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_dot: null output");
     const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
     return rs_launch_block_reduce(m, (const double *)a, (const double *)b, nullptr, nst * lanes, lanes, 1, lanes == 2 ? 1 : 0,
                                   (double *)out_dev, (cudaStream_t)stream);
@@ -100,9 +100,9 @@ extern "C" rs_status rs_block_dot(const rs_mesh *m, const void *a, const void *b
 extern "C" rs_status rs_block_expectation(const rs_mesh *m, const void *psi, const void *hpsi, const double *eps_dev, int nst,
                                           rs_dtype dtype, double *out_dev, void *stream)
 {
+    if (!out_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_expectation: null output");
     rs_status st = check_blocks(m, psi, hpsi, nst, dtype, "rs_block_expectation");
     if (st != RS_OK) return st;
-    if (!out_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_expectation: null output");
     const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
     return rs_launch_block_reduce(m, (const double *)psi, (const double *)hpsi, eps_dev, nst * lanes, lanes, 3, 0, out_dev,
                                   (cudaStream_t)stream);
@@ -110,9 +110,9 @@ extern "C" rs_status rs_block_expectation(const rs_mesh *m, const void *psi, con
 
 extern "C" rs_status rs_block_axpy(const rs_mesh *m, const void *alpha_dev, const void *x, void *y, int nst, rs_dtype dtype, void *stream)
 {
+    if (!alpha_dev || x == y) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_axpy: null alpha or x == y");
     rs_status st = check_blocks(m, x, y, nst, dtype, "rs_block_axpy");
     if (st != RS_OK) return st;
-    if (!alpha_dev || x == y) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_axpy: null alpha or x == y");
     const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
     return rs_launch_block_axpy(m, (const double *)alpha_dev, (const double *)x, (double *)y, nst * lanes, lanes, (cudaStream_t)stream);
 }
@@ -128,9 +128,9 @@ extern "C" rs_status rs_block_copy(const rs_mesh *m, const void *src, void *dst,
 // ---- f2: overlap / subspace matrices over blocks of points (eqs. 5 and 7) -----------------------
 extern "C" rs_status rs_block_overlap(const rs_mesh *m, const void *a, const void *b, int nst, rs_dtype dtype, void *M_dev, void *stream)
 {
+    if (!M_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_overlap: null output");
     rs_status st = check_blocks(m, a, b, nst, dtype, "rs_block_overlap");
     if (st != RS_OK) return st;
-    if (!M_dev) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_overlap: null output");
     const int lanes = dtype == RS_COMPLEX128 ? 2 : 1;
     if (nst * lanes == 1)   // a single real column: the 1 x 1 matrix is the dot product
         return rs_launch_block_reduce(m, (const double *)a, (const double *)b, nullptr, 1, 1, 1, 0, (double *)M_dev, (cudaStream_t)stream);

@@ -32,7 +32,8 @@ def test_binding_never_imports_oracle():
     assert "oracle" not in src
     for f in os.listdir(os.path.join(ROOT, "paper_1306_2953_b200", "csrc")):
         assert "oracle" not in open(os.path.join(ROOT, "paper_1306_2953_b200", "csrc", f)).read().lower(), f
-    osrc = open(os.path.join(ROOT, "oracle", "oracle.c")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    osrc = (open(os.path.join(ROOT, "oracle", "oracle.c")).read() + open(os.path.join(ROOT, "oracle", "oracle_next.c")).read() +
+            open(os.path.join(ROOT, "oracle", "__init__.py")).read())
     assert "rs.h" not in osrc and "import paper_1306" not in osrc and "librs" not in osrc
 
 
@@ -320,4 +321,49 @@ def test_nonlocal_spheres_equal_the_oracles_and_colours_are_race_free():
     assert far.ncolors == 1 and far.sphere(1).size == 0 and far.sphere(0).size > 0
     with pytest.raises(rs.RsError) as e:
         rs.rs_nonlocal_create(mesh, cfg.centers, rc, 17)
+    assert e.value.status == rs.RS_ERR_INVALID_ARG
+
+
+def test_next_row_entry_points_check_arguments_without_a_device():
+    """f1-f3 entry points: bad arguments -> RS_ERR_INVALID_ARG, good arguments on a host-only handle -> RS_ERR_CUDA (no fallback)."""
+    import ctypes as C
+
+    m = rs.rs_mesh_create_box(8, 8, 8, 0.25, 4)
+    npts = m.npoints
+
+    def aligned(n):
+        raw = np.zeros(n + 2)
+        return raw[(0 if raw.ctypes.data % 16 == 0 else 1):][:n]
+
+    a, b = aligned((npts + 1) * 4), aligned((npts + 1) * 4)
+    out = np.zeros(16)
+    L, h = rs._lib, m.handle
+    ptr = lambda x: C.c_void_p(x.ctypes.data)
+    assert L.rs_block_dot(h, ptr(a), ptr(b), 3, rs.RS_REAL64, ptr(out), None) == rs.RS_ERR_INVALID_ARG          # width not a power of two
+    assert L.rs_block_dot(h, ptr(a), None, 4, rs.RS_REAL64, ptr(out), None) == rs.RS_ERR_INVALID_ARG
+    assert L.rs_block_dot(h, ptr(a[1:]), ptr(b), 4, rs.RS_REAL64, ptr(out), None) == rs.RS_ERR_INVALID_ARG      # misaligned block
+    assert L.rs_block_axpy(h, ptr(out), ptr(a), ptr(a), 4, rs.RS_REAL64, None) == rs.RS_ERR_INVALID_ARG         # x == y
+    assert L.rs_block_overlap(h, ptr(a), ptr(b), 4, 7, ptr(out), None) == rs.RS_ERR_INVALID_ARG                 # bad dtype
+    assert L.rs_block_expectation(h, ptr(a), ptr(b), None, 4, rs.RS_REAL64, None, None) == rs.RS_ERR_INVALID_ARG
+    c = np.array([-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560])
+    assert L.rs_hamiltonian_apply_ex(h, 4, c.ctypes.data_as(C.POINTER(C.c_double)), ptr(out), ptr(a), ptr(b), 4, rs.RS_REAL64, None,
+                                     None, None) == rs.RS_ERR_INVALID_ARG
+    import torch
+    if not torch.cuda.is_available():
+        for call in (lambda: L.rs_block_dot(h, ptr(a), ptr(b), 4, rs.RS_REAL64, ptr(out), None),
+                     lambda: L.rs_block_overlap(h, ptr(a), ptr(b), 4, rs.RS_REAL64, ptr(out), None),
+                     lambda: L.rs_block_axpy(h, ptr(out), ptr(a), ptr(b), 4, rs.RS_REAL64, None),
+                     lambda: L.rs_block_copy(h, ptr(a), ptr(b), 4, rs.RS_REAL64, None),
+                     lambda: L.rs_hamiltonian_prepare(h, 4, 4, rs.RS_REAL64)):
+            assert call() == rs.RS_ERR_CUDA
+        nl = rs.rs_nonlocal_create(m, np.zeros((1, 3)), 0.6, 1)
+        nl.set_projectors(0, np.ones((nl.sphere(0).size, 1)))
+        with pytest.raises(rs.RsError) as e:
+            rs.rs_nonlocal_apply(nl, a, b, 4, stream=0)
+        assert e.value.status == rs.RS_ERR_CUDA
+        with pytest.raises(rs.RsError) as e:
+            rs.rs_workspace_create(m, 4, rs.RS_REAL64, npts)
+        assert e.value.status == rs.RS_ERR_CUDA
+    with pytest.raises(rs.RsError) as e:
+        rs.rs_workspace_create(m, 4, rs.RS_REAL64, npts - 1)            # ld < np
     assert e.value.status == rs.RS_ERR_INVALID_ARG
