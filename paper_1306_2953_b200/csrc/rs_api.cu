@@ -373,6 +373,7 @@ extern "C" rs_status rs_mesh_set_sweep_options(rs_mesh *m, const rs_sweep_option
         rs_sweep_free(m);
     }
     m->sweep_costs.clear();
+    m->sweep_pieces.clear();
     m->opt = *opt;
     return RS_OK;
 }

@@ -30,6 +30,8 @@ constexpr int RS_BRICK_PTS = RS_BRICK * RS_BRICK * RS_BRICK;  // 64 points
 #define RS_SWEEP_MAXRUN 64
 struct rs_sweep_piece {
     int iy, iz, xa, xb, chunk;   // tile, output planes [xa, xb), column slice
+    bool operator==(const rs_sweep_piece &o) const { return iy == o.iy && iz == o.iz && xa == o.xa && xb == o.xb && chunk == o.chunk; }
+    bool operator!=(const rs_sweep_piece &o) const { return !(*this == o); }
 };
 struct rs_sweep_host {
     std::vector<int2> items;                         // per CTA: {first record, number of steps}
@@ -58,6 +60,7 @@ struct rs_sweep_tables {
     std::vector<int2> host_items;                    // copies kept for rs_hamiltonian_autotune
     std::vector<int32_t> rec_cell;
     std::vector<int64_t> host_stats;                 // per CTA: {steps, pieces, modelled load x 1000, full warp-steps}
+    std::vector<std::vector<rs_sweep_piece>> pieces; // the dealing these tables were built from (refined by rs_hamiltonian_autotune)
 };
 
 // encoded tensor maps of one psi buffer (rs_sweep.cu: 6 CUtensorMap of 128 bytes), kept per (pointer, row pitch)
@@ -89,6 +92,7 @@ struct rs_mesh {
     int32_t *d_map[RS_MAX_FD_ORDER + 1] = {nullptr};                 // [np][6n], built lazily per order
     std::map<std::pair<int, int>, rs_sweep_tables> sweep;            // (fd_order, ncol) -> tables, built lazily
     std::map<std::pair<int, int>, rs_sweep_costs> sweep_costs;       // measured step costs, if autotuned
+    std::map<std::pair<int, int>, std::vector<std::vector<rs_sweep_piece>>> sweep_pieces;   // a refined dealing that replaces the dealt one
     std::vector<rs_sweep_map_cache> map_cache;                       // tensor maps per psi buffer (blocks wider than 16 columns)
     rs_sweep_options opt = {32, 1 << 20, 0, 0, 3, 3};                // rs_mesh_set_sweep_options
     double *d_red = nullptr;                                         // per-CTA partial sums of the block reductions (rs_blas.cu)
@@ -135,7 +139,8 @@ const char *rs_sweep_variant_name(const rs_mesh *m, int n, int ncol);
 void rs_sweep_free(rs_mesh *m);
 // host-only construction of the records; false if a plane needs more than RS_SWEEP_MAXRUN runs
 bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int nctas, rs_sweep_host &out,
-                         const rs_sweep_costs *measured = nullptr);
+                         const rs_sweep_costs *measured = nullptr,
+                         const std::vector<std::vector<rs_sweep_piece>> *given_pieces = nullptr);
 rs_status rs_sweep_prepare(const rs_mesh *m, int n, int ncol);   // build + upload the tables now
 rs_status rs_sweep_autotune(const rs_mesh *m, int n, const rs_weights &w, const double *vloc, const double *psi, double *hpsi,
                             int ncol, cudaStream_t st);
