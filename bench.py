@@ -196,6 +196,66 @@ def traffic_rows() -> dict:
     return {row["key"]: row for row in csv.DictReader(open(path))}
 
 
+def run_streamed(args) -> None:
+    """BASELINE.json configs[4] at its stated size: the whole orbital set streamed through HBM block by block from HOST memory
+    (rs_hamiltonian_apply_states_stream, 3-window workspace).  Orbitals are generated chunk by chunk into one pinned buffer, so
+    neither side ever holds the set (31 GB for config 4); generation time is not timed; one seeded orbital per chunk is compared
+    with the oracle.  Prints one JSON line (an e2e-only record, not the driver's bench line)."""
+    import torch
+
+    import oracle
+    import paper_1306_2953_b200 as rs
+
+    cfg = synthetic.config(args.config)
+    n = args.fd_order or cfg.fd_orders[0]
+    B, chunk = args.block, args.stream_chunk
+    nst = args.nst or cfg.nst
+    is_c = cfg.is_complex
+    tdt = torch.complex128 if is_c else torch.float64
+    rsdt = rs.RS_COMPLEX128 if is_c else rs.RS_REAL64
+    torch.cuda.set_device(0)
+    mesh = rs.rs_mesh_create(cfg.centers, cfg.radius, cfg.spacing, max(cfg.fd_orders))
+    npts = mesh.npoints
+    ijk = mesh.points()
+    rank_of = synthetic.canonical_rank(ijk)
+    om = oracle.mesh_from_spheres(cfg.centers, cfg.radius, cfg.spacing)
+    vc = synthetic.vloc_at(om.xyz(), cfg.centers, cfg.charges)
+    host_v = torch.from_numpy(np.ascontiguousarray(vc[rank_of])).pin_memory()
+    host_in = torch.empty((chunk, npts), dtype=tdt).pin_memory()
+    host_out = torch.empty((chunk, npts), dtype=tdt).pin_memory()
+    coeffs = fd_coeffs(n)
+    ws = rs.rs_workspace_create(mesh, B, rsdt, npts)
+    rng = np.random.default_rng(args.config)
+    total, worst, checked = 0.0, 0.0, []
+    for ist0 in range(0, nst, chunk):
+        nb = min(chunk, nst - ist0)
+        hin = host_in.numpy()
+        for j in range(nb):
+            hin[j] = synthetic.orbital(cfg.seed, ist0 + j, npts, is_c)[rank_of]
+        if ist0 == 0:   # warm-up (tables, first touch of the pinned buffers), not timed
+            rs.rs_hamiltonian_apply_states_stream(ws, n, coeffs, host_v, host_in[:nb], host_out[:nb])
+        torch.cuda.synchronize()
+        t = time.perf_counter()
+        rs.rs_hamiltonian_apply_states_stream(ws, n, coeffs, host_v, host_in[:nb], host_out[:nb])
+        total += time.perf_counter() - t
+        j = int(rng.integers(0, nb))
+        psi = synthetic.orbital(cfg.seed, ist0 + j, npts, is_c)[None, :]
+        o = oracle.hpsi(om, n, oracle.fd_coeffs(n), vc, psi, nthreads=len(os.sched_getaffinity(0)))
+        g = np.empty_like(o)
+        g[:, rank_of] = host_out.numpy()[j:j + 1]
+        err = float(np.abs(g - o).max() / np.abs(o).max())
+        worst = err if not (err <= worst) else worst          # a NaN must not hide behind max()
+        checked.append(ist0 + j)
+    esz = 16 if is_c else 8
+    fl = nst * npts * flops_per_output(n) * (4 if is_c else 1)
+    print(json.dumps({"metric": METRIC, "impl": "ours-streamed", "value": fl / total / 1e9, "unit": UNIT, "seconds": total,
+                      "config": workload_config(cfg, n, B, npts, nst), "chunk_orbitals": chunk,
+                      "h2d_bytes": nst * npts * esz + (nst + chunk - 1) // chunk * npts * 8, "d2h_bytes": nst * npts * esz,
+                      "gbs_per_direction": nst * npts * esz / total / 1e9, "workspace_bytes": ws.nbytes,
+                      "device_resident_states_bytes": 0, "max_normwise_err": worst, "checked_orbitals": checked,
+                      "api": "rs_hamiltonian_apply_states_stream, one call per chunk, pinned host buffers"}))
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -217,9 +277,15 @@ def main() -> None:
     ap.add_argument("--planes-tuned", type=int, default=0,
                     help="x-slab thickness of the plane-sweep work pieces after autotune (0: library default = whole tile columns)")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the timings of the f1-f3 operations (SURVEY.md 8(f))")
+    ap.add_argument("--stream-chunk", type=int, default=0,
+                    help="e2e only, for orbital sets too large to keep resident: stream the config's orbitals from host memory in "
+                         "chunks of this many, generated on the fly (configs[4]: 1024 orbitals)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.stream_chunk:
+        run_streamed(args)
         return
 
     import torch
