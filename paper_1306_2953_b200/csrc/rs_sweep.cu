@@ -1335,6 +1335,15 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
     bool best_is_model = true, cur_is_model = m->sweep_costs.find(key) == m->sweep_costs.end();
     rs_sweep_costs best_costs, cur_costs;
     if (!cur_is_model) cur_costs = m->sweep_costs[key];
+    // drop the device tables: the next use builds them again (from the costs / pieces then in the handle)
+    auto drop_tables = [&]() {
+        auto f = m->sweep.find(key);
+        if (f != m->sweep.end()) {
+            rs_sweep_tables &t = f->second;
+            cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles), cudaFree(t.d_step_clock);
+            m->sweep.erase(f);
+        }
+    };
     auto slowest_cta = [&](const rs_sweep_tables *tb, long long *out) -> rs_status {
         std::vector<long long> cyc((size_t)tb->nitems);
         RS_CUDA_TRY(cudaMemcpy(cyc.data(), tb->d_cycles, cyc.size() * sizeof(long long), cudaMemcpyDeviceToHost));
@@ -1359,8 +1368,6 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
         }
         std::vector<long long> clk((size_t)tb->nrec + 1);
         RS_CUDA_TRY(cudaMemcpy(clk.data(), tb->d_step_clock, clk.size() * sizeof(long long), cudaMemcpyDeviceToHost));
-        size_t ncell = 0;
-        for (int32_t c : tb->rec_cell) ncell = std::max(ncell, (size_t)(c + 1));
         const shape_rt sh = variant_shape(tb->variant);
         const size_t cells = (size_t)((m->dims[1] + sh.TY - 1) / sh.TY) * ((m->dims[2] + SW_TZ - 1) / SW_TZ) * m->dims[0];
         std::vector<double> sum(cells, 0.0);
@@ -1387,24 +1394,10 @@ rs_status rs_sweep_autotune(const rs_mesh *cm, int n, const rs_weights &w, const
         costs.unit = full_sum / full_n;
         m->sweep_costs[key] = costs;
         cur_costs = costs, cur_is_model = false;
-        // drop the tables: the next use builds them with the measured costs
-        auto f = m->sweep.find(key);
-        if (f != m->sweep.end()) {
-            rs_sweep_tables &t = f->second;
-            cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles), cudaFree(t.d_step_clock);
-            m->sweep.erase(f);
-        }
+        drop_tables();   // the next use builds them with the measured costs
     }
     // if an earlier dealing was faster than the last one, go back to it
-    auto drop_tables = [&]() {
-        auto f = m->sweep.find(key);
-        if (f != m->sweep.end()) {
-            rs_sweep_tables &t = f->second;
-            cudaFree(t.d_items), cudaFree(t.d_recs), cudaFree(t.d_cycles), cudaFree(t.d_step_clock);
-            m->sweep.erase(f);
-        }
-    };
-    auto measure = [&](std::vector<long long> &cyc, const rs_sweep_tables **tbo) -> rs_status {   // 3 launches; the last one's per-CTA clocks
+    auto measure = [&](std::vector<long long> &cyc, const rs_sweep_tables **tbo) -> rs_status {   // per-CTA clocks, mean of 3 launches
         const rs_sweep_tables *tb = nullptr;
         rs_status rc = get_tables(m, n, ncol, &tb);
         if (rc != RS_OK) return rc;
