@@ -203,7 +203,9 @@ rs_status rs_hamiltonian_prepare(const rs_mesh *mesh, int fd_order, int nst, rs_
 /* Optional, once per (mesh, fd_order, nst, dtype): "measure, don't guess".  Runs the kernel a few times on the
  * caller's buffers (arguments as rs_hamiltonian_apply; hpsi receives H psi), reads back the clock each persistent
  * CTA recorded at the end of every plane, and deals the work to the CTAs again using the measured cost of every
- * (tile, plane) instead of the built-in cost model.  Later rs_hamiltonian_apply calls use the re-dealt tables; results
+ * (tile, plane) instead of the built-in cost model, then refines that dealing by moving the planes at which a tile column is
+ * split between two CTAs towards the slower one; the fastest dealing measured is kept (about 0.5-1 s once per mesh, order and
+ * width).  Later rs_hamiltonian_apply calls use the re-dealt tables; results
  * are unchanged up to rounding order.  SYNCHRONISES `stream` and replaces the mesh's device tables: no other call
  * on this mesh may be in flight on another stream or thread.  A call that only the gather kernel can serve is just
  * applied.                                                                                                        */
@@ -253,7 +255,8 @@ typedef struct {
     int ctas;          /* persistent CTAs (0 = one per SM)                                                          */
     int force_tensor;  /* 1 = use the 2-D tensor-map copies also for 16-column blocks                               */
     int min_split;     /* fewest output planes of a work piece cut off when dealing (default 3)                     */
-    int tune_rounds;   /* measure / re-deal rounds of rs_hamiltonian_autotune (default 3)                           */
+    int tune_rounds;   /* measure / re-deal rounds of rs_hamiltonian_autotune (default 3); it then runs up to twice as
+                          many refinement rounds that only move the split planes of shared tile columns               */
 } rs_sweep_options;
 rs_status rs_sweep_options_default(rs_sweep_options *out);
 rs_status rs_mesh_set_sweep_options(rs_mesh *mesh, const rs_sweep_options *opt);
