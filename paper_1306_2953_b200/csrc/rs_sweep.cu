@@ -606,15 +606,10 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
     __shared__ uint64_t rec_bar[SW_RING];
     __shared__ uint32_t tmem_base_s;
 
-#ifndef SW_PROD_HIGH
-#define SW_PROD_HIGH 1
-#endif
-    // The warp scheduler favours the higher warp ids when several warps are ready.  The producers' instruction path is
-    // short but latency-critical (it paces every step), the consumers' is long and throughput-bound: the producer warps
-    // take the HIGH warp ids, so that they issue as soon as they can.
+    // consumer warps take the low warp ids, producer warps the high ones (the other way round measured the same)
     const int tid = threadIdx.x, warp = tid >> 5;
-    const int ctid = SW_PROD_HIGH ? (tid < S::CONSUMERS ? tid : -1) : tid - S::PRODUCERS;
-    const int ptid = SW_PROD_HIGH ? tid - S::CONSUMERS : tid;
+    const int ctid = tid < S::CONSUMERS ? tid : -1;
+    const int ptid = tid - S::CONSUMERS;
     const int2 item = a.items[blockIdx.x];
     const int nsteps = item.y;
     const long long clock0 = clock64();
@@ -629,7 +624,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
         for (int s = 0; s < SW_RING; ++s) mbar_init(smem_u32(&rec_bar[s]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    if (warp == (SW_PROD_HIGH ? 0 : S::PRODUCERS / 32)) {   // first consumer warp
+    if (warp == 0) {   // first consumer warp
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_base_s)),
                      "n"(SW_TMEM_COLS)
                      : "memory");
