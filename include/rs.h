@@ -173,14 +173,19 @@ rs_status rs_hamiltonian_apply_ex(const rs_mesh *mesh, int fd_order, const doubl
 
 /* ---- non-local potential (sec. V.C, eq. 4 at :181) -------------------------------
  *   hpsi[r][j] += sum_A sum_lm gamma^A_lm(r - R_A) * h^3 sum_{r' in sphere A} gamma^A_lm(r' - R_A) psi[r'][j]
- * in the paper's two parts: the projection integrals are computed and stored, then multiplied by the projectors and
- * added, atoms grouped into colours whose spheres share no mesh point so that each colour is one race-free launch
- * (Fig. 11).  The sphere of atom A is the closed ball |r - R_A| <= rc restricted to the mesh.
+ * in the paper's two parts: the projection integrals are computed and stored, then multiplied by
+ * the projectors and added.  The paper parallelises part 2 over atoms and therefore groups the atoms into colours whose
+ * spheres share no mesh point (Fig. 11); here part 2 is a gather over the union of the spheres (every covered mesh point
+ * adds up the atoms that cover it and is written once), which needs no colours and one launch.  The colouring is still
+ * computed and published (rs_nonlocal_ncolors / rs_nonlocal_get_colors) for callers that scatter by atom themselves.
+ * The sphere of atom A is the closed ball |r - R_A| <= rc restricted to the mesh (it may be empty).
  * The projector VALUES are an input (pseudopotential data, real): after rs_nonlocal_create the caller reads each atom's
  * sphere points (rs_nonlocal_sphere_size / rs_nonlocal_get_sphere: mesh indices, ascending), samples its nlm projectors
  * there and hands them over with rs_nonlocal_set_projectors (host [npts_A][nlm]).  nlm <= 16 (l_max = 3).
  * rs_nonlocal_apply ACCUMULATES into hpsi (call it after rs_hamiltonian_apply); asynchronous on `stream`; the first
  * call uploads the tables (rs_nonlocal_prepare does that ahead of time); deterministic (fixed-order sums, no atomics).
+ * psi_dev / hpsi_dev: blocks of the mesh, 16-byte aligned, distinct.  Three kernels per call, chained by programmatic
+ * dependent launch inside the call; to the rest of the stream the call behaves like one kernel.
  * The handle keeps per-call scratch: one apply at a time per handle.  The mesh must outlive the handle.           */
 typedef struct rs_nonlocal rs_nonlocal; /* opaque */
 rs_status rs_nonlocal_create(const rs_mesh *mesh, const double *centers_host, int natoms, double rc, int nlm,

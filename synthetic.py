@@ -115,8 +115,8 @@ def vloc_at(xyz: np.ndarray, centers: np.ndarray, charges: np.ndarray, chunk: in
 
 def projector_values(xyz_rel: np.ndarray, lmax: int = 1, sigma: float = 0.7) -> np.ndarray:
     """Synthetic stand-ins for the pseudopotential projectors gamma_lm(r - R_A) of PAPER.md:181 (eq. 4), whose real
-    data are not available: a Gaussian exp(-r^2/(2 sigma^2)) times the real solid harmonics up to lmax <= 2
-    (1; x, y, z; xy, yz, zx, x^2-y^2, 3z^2-r^2).  An INPUT of the path, sampled at caller-supplied coordinates
+    data are not available: a Gaussian exp(-r^2/(2 sigma^2)) times the real solid harmonics up to lmax <= 3
+    (1; x, y, z; xy, yz, zx, x^2-y^2, 3z^2-r^2; the seven cubic ones), unnormalised.  An INPUT of the path, sampled at caller-supplied coordinates
     relative to the atom; the caller decides which points lie inside the cut-off sphere.  Returns [n][(lmax+1)^2]."""
     p = np.ascontiguousarray(xyz_rel, dtype=np.float64).reshape(-1, 3)
     x, y, z = p[:, 0], p[:, 1], p[:, 2]
@@ -127,8 +127,11 @@ def projector_values(xyz_rel: np.ndarray, lmax: int = 1, sigma: float = 0.7) -> 
         cols += [x, y, z]
     if lmax >= 2:
         cols += [x * y, y * z, z * x, x * x - y * y, 3.0 * z * z - r2]
-    if lmax > 2:
-        raise ValueError("lmax <= 2")
+    if lmax >= 3:
+        cols += [z * (5.0 * z * z - 3.0 * r2), x * (5.0 * z * z - r2), y * (5.0 * z * z - r2), z * (x * x - y * y), x * y * z,
+                 x * (x * x - 3.0 * y * y), y * (3.0 * x * x - y * y)]
+    if lmax > 3:
+        raise ValueError("lmax <= 3")
     return np.stack(cols, axis=1) * g[:, None]
 
 

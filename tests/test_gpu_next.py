@@ -185,9 +185,10 @@ def test_subspace_hamiltonian_of_plane_waves_is_diagonal():
 
 
 # ---- f3 ----------------------------------------------------------------------------------------------------------
-def make_nonlocal(p, centers, rc, lmax, sigma=0.7):
+def make_nonlocal(p, centers, rc, lmax, sigma=0.7, oracle_atoms=None):
     """The same INPUT (synthetic.projector_values) on both sides: the library samples it at the sphere points it
-    publishes, the oracle at its own; the two point sets are compared first."""
+    publishes, the oracle at its own; the two point sets are compared first.  oracle_atoms: the atoms the oracle is
+    given (an atom whose sphere holds no mesh point adds nothing to eq. 4, and the oracle's helper wants >= 1 point)."""
     nlm = (lmax + 1) ** 2
     nl = rs.rs_nonlocal_create(p.mesh, centers, rc, nlm)
     h = p.mesh.spacing
@@ -195,7 +196,8 @@ def make_nonlocal(p, centers, rc, lmax, sigma=0.7):
         idx = nl.sphere(A)
         assert np.array_equal(np.sort(p.rank[idx]), oracle.sphere_points(p.omesh, centers[A], rc))
         nl.set_projectors(A, synthetic.projector_values(p.ijk[idx].astype(np.float64) * h - centers[A], lmax, sigma))
-    proj = oracle.make_projectors(p.omesh, centers, rc, lambda x: synthetic.projector_values(x, lmax, sigma))
+    oc = centers if oracle_atoms is None else centers[oracle_atoms]
+    proj = oracle.make_projectors(p.omesh, oc, rc, lambda x: synthetic.projector_values(x, lmax, sigma))
     return nl, proj
 
 
@@ -225,6 +227,33 @@ def test_nonlocal_apply_matches_the_oracle(B, nst, is_complex, lmax):
     rs.rs_nonlocal_apply(nl, blk, hb2, B)
     assert torch.equal(hblk, hb2)                                   # deterministic
     assert torch.all(hblk[p.np] == 0)
+
+
+@pytest.mark.parametrize("lmax", [0, 3])
+def test_nonlocal_crowded_and_empty_spheres(lmax):
+    """Five atoms within one bohr of each other (up to five spheres over one point: the further-pairs path of the
+    gather), an atom whose sphere misses the mesh, one at the mesh edge; large spheres (many chunks per atom, the
+    persistent CTAs of part 1 change atom in mid-range); 1 and 16 projectors; one handle reused at several widths."""
+    import torch
+
+    p = problem(1)
+    c0 = p.cfg.centers[0]
+    rng = np.random.default_rng(7)
+    centers = np.concatenate([c0 + rng.uniform(-0.5, 0.5, (5, 3)), [c0 + 60.0], [p.cfg.centers[-1] + [p.cfg.radius * 0.9, 0.0, 0.0]]])
+    nl, proj = make_nonlocal(p, centers, 3.0, lmax, sigma=1.1, oracle_atoms=[0, 1, 2, 3, 4, 6])
+    assert nl.sphere(5).size == 0 and nl.sphere(0).size > 5000
+    for B, nst, is_complex in ((1, 1, False), (2, 2, False), (16, 16, False), (8, 8, True), (64, 33, False)):
+        psi = rand_orbitals(50 + B, nst, p.np, is_complex)
+        base = rand_orbitals(51 + B, nst, p.np, is_complex)
+        blk, hblk = to_block(p, psi, B), to_block(p, base, B)
+        rs.rs_nonlocal_apply(nl, blk, hblk, B)
+        g = from_block(p, hblk, nst)
+        o = oracle.nonlocal_apply(p.omesh, proj, psi, base)
+        vn = oracle.nonlocal_apply(p.omesh, proj, np.abs(psi.real) + (np.abs(psi.imag) if is_complex else 0.0))
+        assert (np.abs(g - o) <= 1e-12 * (np.abs(vn).max() + np.abs(base))).all(), (B, nst)
+        hb2 = to_block(p, base, B)
+        rs.rs_nonlocal_apply(nl, blk, hb2, B)
+        assert torch.equal(hblk, hb2)
 
 
 def test_full_hamiltonian_with_nonlocal_term_is_hermitian_on_gpu():

@@ -348,6 +348,10 @@ def test_next_row_entry_points_check_arguments_without_a_device():
     c = np.array([-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560])
     assert L.rs_hamiltonian_apply_ex(h, 4, c.ctypes.data_as(C.POINTER(C.c_double)), ptr(out), ptr(a), ptr(b), 4, rs.RS_REAL64, None,
                                      None, None) == rs.RS_ERR_INVALID_ARG
+    nl0 = rs.rs_nonlocal_create(m, np.zeros((1, 3)), 0.6, 1)
+    nl0.set_projectors(0, np.ones((nl0.sphere(0).size, 1)))
+    assert L.rs_nonlocal_apply(nl0._h, ptr(a[1:]), ptr(b), 4, rs.RS_REAL64, None) == rs.RS_ERR_INVALID_ARG      # misaligned block
+    assert L.rs_nonlocal_apply(nl0._h, ptr(a), ptr(a), 4, rs.RS_REAL64, None) == rs.RS_ERR_INVALID_ARG          # in place
     import torch
     if not torch.cuda.is_available():
         for call in (lambda: L.rs_block_dot(h, ptr(a), ptr(b), 4, rs.RS_REAL64, ptr(out), None),
