@@ -8,7 +8,7 @@
 //
 // This is the one dense contraction on the path, so it runs on the fp64 tensor-core path: mma.sync m8n8k4 (DMMA),
 // hand-written (no cuBLAS).  tcgen05 has no fp64 kind, so DMMA is what sm_100a offers for this arithmetic type.
-//   * persistent CTAs (one per SM), each streaming its tiles of P points through a 3-stage cp.async ring;
+//   * persistent CTAs (one to three per SM), each streaming its tiles of P points through a 3-stage cp.async ring;
 //   * 8 warps: the (C/8)^2 output tiles of 8 x 8 are split into warp blocks of MT x NT tiles, the remaining
 //     factor of 8 splits the points of a tile (K slices); row pitch padded to 4 (mod 16) doubles: the DMMA fragment
 //     loads (lane -> point lane % 4, column lane / 4) are bank-conflict free;
@@ -24,13 +24,18 @@ template <int C_>
 struct ov_shape {
     static constexpr int C = C_;                                        // real columns, padded to >= 8
     static constexpr int MT = C <= 8 ? 1 : C == 16 ? 2 : 4;             // 8 x 8 tiles per warp (rows)
-    static constexpr int NT = C <= 8 ? 1 : C == 16 ? 2 : C == 32 ? 4 : 8;
+    static constexpr int NT = C <= 8 ? 1 : C == 16 ? 2 : C <= 64 ? 4 : 8;
     static constexpr int WM = C / 8 / MT, WN = C / 8 / NT;              // warp blocks
     static constexpr int KS = 8 / (WM * WN);                            // K slices
-    static constexpr int P = C <= 32 ? 128 : C == 64 ? 64 : 32;         // points per stage
+    // points per stage / stages / CTAs per SM.  Blocks of <= 32 columns are bandwidth-bound and their tiles are small:
+    // two or three CTAs per SM (independent barriers) keep more copies in flight than one CTA with a deeper ring
+    // (measured, config 2: B = 16 0.120 -> 0.091 ms, B = 32 0.263 -> 0.185 ms); 64 columns: 32 x 32 warp blocks on two
+    // CTAs per SM (0.73 -> 0.62 ms); 128 columns are bound by the DMMA rate.
+    static constexpr int P = C <= 32 ? 64 : 32;
+    static constexpr int STAGES = 3;
+    static constexpr int CPS = C <= 16 ? 3 : C <= 64 ? 2 : 1;
     static constexpr int PITCH = C % 16 == 0 ? C + 4 : C == 8 ? 12 : 4; // doubles; = 4 or 12 (mod 16)
     static constexpr int TILE = P * PITCH;                              // doubles per operand per stage
-    static constexpr int STAGES = C <= 16 ? 5 : 3;                      // narrow blocks: small tiles, more of them in flight
     static constexpr size_t SMEM_RING = (size_t)STAGES * 2 * TILE * 8;
     static constexpr size_t SMEM_RED = (size_t)KS * C * C * 8;
     static constexpr size_t SMEM = SMEM_RING > SMEM_RED ? SMEM_RING : SMEM_RED;
@@ -52,7 +57,7 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
 
 // x, y: blocks [np + 1][cr] (cr real columns, cr <= C; columns cr..C-1 of the shared tiles stay zero).  same = (x == y).
 template <class S>
-__global__ void __launch_bounds__(OV_THREADS, 1) overlap_kernel(const double *__restrict__ x, const double *__restrict__ y, int64_t np,
+__global__ void __launch_bounds__(OV_THREADS, S::CPS) overlap_kernel(const double *__restrict__ x, const double *__restrict__ y, int64_t np,
                                                                 int cr, int same, double *__restrict__ partial)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -137,24 +142,34 @@ __global__ void __launch_bounds__(OV_THREADS, 1) overlap_kernel(const double *__
     }
 }
 
-// M[j][k], j, k < nst: real: sum_cta G[j][k]; complex: (G[2j][2k] + G[2j+1][2k+1]) + i (G[2j][2k+1] - G[2j+1][2k])
-__global__ void overlap_final_kernel(const double *__restrict__ partial, int nctas, int C, int nst, int lanes, double *__restrict__ M)
+// M[j][k], j, k < nst: real: sum_cta G[j][k]; complex: (G[2j][2k] + G[2j+1][2k+1]) + i (G[2j][2k+1] - G[2j+1][2k]).
+// One warp per entry: lane l adds the CTAs l, l + 32, ... in order, then a butterfly over the lanes: a fixed order
+// (deterministic) without a serial walk over all CTAs.
+__global__ void __launch_bounds__(256) overlap_final_kernel(const double *__restrict__ partial, int nctas, int C, int nst, int lanes,
+                                                           double *__restrict__ M)
 {
-    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nst * nst; idx += gridDim.x * blockDim.x) {
-        const int j = idx / nst, k = idx % nst;
-        if (lanes == 1) {
-            double s = 0.0;
-            for (int c = 0; c < nctas; ++c) s += partial[(size_t)c * C * C + j * C + k];
-            M[idx] = s;
-        } else {
-            double re = 0.0, im = 0.0;
-            for (int c = 0; c < nctas; ++c) {
-                const double *G = partial + (size_t)c * C * C;
-                re += G[(2 * j) * C + 2 * k] + G[(2 * j + 1) * C + 2 * k + 1];
-                im += G[(2 * j) * C + 2 * k + 1] - G[(2 * j + 1) * C + 2 * k];
-            }
-            M[2 * idx] = re, M[2 * idx + 1] = im;
+    const int lane = threadIdx.x & 31;
+    const int idx = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (idx >= nst * nst) return;
+    const int j = idx / nst, k = idx % nst;
+    double re = 0.0, im = 0.0;
+    if (lanes == 1) {
+        for (int c = lane; c < nctas; c += 32) re += partial[(size_t)c * C * C + j * C + k];
+    } else {
+        for (int c = lane; c < nctas; c += 32) {
+            const double *G = partial + (size_t)c * C * C;
+            re += G[(2 * j) * C + 2 * k] + G[(2 * j + 1) * C + 2 * k + 1];
+            im += G[(2 * j) * C + 2 * k + 1] - G[(2 * j + 1) * C + 2 * k];
         }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        re += __shfl_xor_sync(0xffffffffu, re, off);
+        im += __shfl_xor_sync(0xffffffffu, im, off);
+    }
+    if (lane == 0) {
+        if (lanes == 1) M[idx] = re;
+        else M[2 * idx] = re, M[2 * idx + 1] = im;
     }
 }
 
@@ -166,7 +181,7 @@ rs_status launch(const rs_mesh *m, const double *x, const double *y, int cr, dou
         RS_CUDA_TRY(cudaFuncSetAttribute(overlap_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM));
         attr_set = true;
     }
-    overlap_kernel<S><<<grid, OV_THREADS, S::SMEM, st>>>(x, y, m->np, cr, x == y ? 1 : 0, partial);
+    overlap_kernel<S><<<grid * S::CPS, OV_THREADS, S::SMEM, st>>>(x, y, m->np, cr, x == y ? 1 : 0, partial);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
 }
@@ -190,16 +205,17 @@ rs_status rs_launch_overlap(const rs_mesh *m, const double *x, const double *y, 
     if (rc != RS_OK) return rc;
     const int nctas = m->sm_count > 0 ? m->sm_count : 148;
     const int C = cr < 8 ? 8 : cr;
+    int cps = 1;
     switch (C) {
-        case 8: rc = launch<ov_shape<8>>(m, x, y, cr, partial, nctas, st); break;
-        case 16: rc = launch<ov_shape<16>>(m, x, y, cr, partial, nctas, st); break;
-        case 32: rc = launch<ov_shape<32>>(m, x, y, cr, partial, nctas, st); break;
-        case 64: rc = launch<ov_shape<64>>(m, x, y, cr, partial, nctas, st); break;
-        case 128: rc = launch<ov_shape<128>>(m, x, y, cr, partial, nctas, st); break;
+        case 8: rc = launch<ov_shape<8>>(m, x, y, cr, partial, nctas, st), cps = ov_shape<8>::CPS; break;
+        case 16: rc = launch<ov_shape<16>>(m, x, y, cr, partial, nctas, st), cps = ov_shape<16>::CPS; break;
+        case 32: rc = launch<ov_shape<32>>(m, x, y, cr, partial, nctas, st), cps = ov_shape<32>::CPS; break;
+        case 64: rc = launch<ov_shape<64>>(m, x, y, cr, partial, nctas, st), cps = ov_shape<64>::CPS; break;
+        case 128: rc = launch<ov_shape<128>>(m, x, y, cr, partial, nctas, st), cps = ov_shape<128>::CPS; break;
         default: return rs_fail(RS_ERR_INVALID_ARG, "rs_block_overlap: block width");
     }
     if (rc != RS_OK) return rc;
-    overlap_final_kernel<<<(cr / lanes * (cr / lanes) + 255) / 256, 256, 0, st>>>(partial, nctas, C, cr / lanes, lanes, M);
+    overlap_final_kernel<<<(cr / lanes * (cr / lanes) + 7) / 8, 256, 0, st>>>(partial, nctas * cps, C, cr / lanes, lanes, M);
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
 }
