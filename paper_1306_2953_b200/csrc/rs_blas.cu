@@ -29,14 +29,7 @@ __global__ void __launch_bounds__(RED_THREADS) block_reduce_kernel(const double 
 #pragma unroll
         for (int v = 0; v < VEC; ++v) e[v] = eps[(col + v) / lanes];
     const int64_t stride = (int64_t)gridDim.x * rpc;
-    for (int64_t ip = (int64_t)blockIdx.x * rpc + prow; ip < np; ip += stride) {
-        double x[VEC], y[VEC];
-        if constexpr (VEC == 2) {
-            const double2 xa = ld2(a + ip * ncol + col), yb = ld2(b + ip * ncol + col);
-            x[0] = xa.x, x[1] = xa.y, y[0] = yb.x, y[1] = yb.y;
-        } else {
-            x[0] = a[ip * ncol + col], y[0] = b[ip * ncol + col];
-        }
+    auto accumulate = [&](const double (&x)[VEC], const double (&y)[VEC]) {
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             acc[0][v] = fma(x[v], y[v], acc[0][v]);
@@ -47,6 +40,35 @@ __global__ void __launch_bounds__(RED_THREADS) block_reduce_kernel(const double 
             }
         }
         if constexpr (CPLX_DOT && VEC == 2) acc[NQ - 1][1] += x[0] * y[1] - x[1] * y[0];   // Im conj(a) b in the im column's last slot
+    };
+    // RED_UNROLL rows per thread in flight (a read-only stream is bound by the bytes in flight, not by the arithmetic);
+    // the rows are still added in ascending order
+    constexpr int RED_UNROLL = 4;
+    int64_t ip = (int64_t)blockIdx.x * rpc + prow;
+    for (; ip + (RED_UNROLL - 1) * stride < np; ip += RED_UNROLL * stride) {
+        double x[RED_UNROLL][VEC], y[RED_UNROLL][VEC];
+#pragma unroll
+        for (int u = 0; u < RED_UNROLL; ++u) {
+            const int64_t o = (ip + u * stride) * ncol + col;
+            if constexpr (VEC == 2) {
+                const double2 xa = ld2(a + o), yb = ld2(b + o);
+                x[u][0] = xa.x, x[u][1] = xa.y, y[u][0] = yb.x, y[u][1] = yb.y;
+            } else {
+                x[u][0] = a[o], y[u][0] = b[o];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < RED_UNROLL; ++u) accumulate(x[u], y[u]);
+    }
+    for (; ip < np; ip += stride) {
+        double x[VEC], y[VEC];
+        if constexpr (VEC == 2) {
+            const double2 xa = ld2(a + ip * ncol + col), yb = ld2(b + ip * ncol + col);
+            x[0] = xa.x, x[1] = xa.y, y[0] = yb.x, y[1] = yb.y;
+        } else {
+            x[0] = a[ip * ncol + col], y[0] = b[ip * ncol + col];
+        }
+        accumulate(x, y);
     }
     // CTA reduction over the rows, fixed order; slot layout partial[cta][q][ncol]
 #pragma unroll
@@ -77,14 +99,25 @@ __global__ void __launch_bounds__(256) block_reduce_final_kernel(const double *_
     if (idx >= nq_out * nst) return;
     const int q = idx / nst, j = idx % nst;
     double s0 = 0.0, s1 = 0.0;
-    if (mode == 1) {
-        for (int c = lane; c < nctas; c += 32) {
-            s0 += partial[((size_t)c * 2 + 0) * ncol + 2 * j] + partial[((size_t)c * 2 + 0) * ncol + 2 * j + 1];
-            s1 += partial[((size_t)c * 2 + 1) * ncol + 2 * j + 1];
+    // eight slots in flight per lane: all loads of a round are issued before the first add (a serial walk costs one
+    // trip to L2 per slot: 37 trips = 25 us, measured), and the adds keep their order
+    for (int c0 = lane; c0 < nctas; c0 += 32 * 8) {
+        double t0[8], t1[8], t2[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int c = c0 + 32 * u;
+            const bool in = c < nctas;
+            const double *p0 = partial + ((size_t)(in ? c : 0) * nq + (mode == 1 ? 0 : q)) * ncol + (size_t)j * lanes;
+            t0[u] = in ? p0[0] : 0.0;
+            t1[u] = in && lanes == 2 ? p0[1] : 0.0;
+            t2[u] = in && mode == 1 ? p0[ncol + 1] : 0.0;       // complex dot: the cross terms in the im column of q1
         }
-    } else {
-        for (int c = lane; c < nctas; c += 32)
-            for (int l = 0; l < lanes; ++l) s0 += partial[((size_t)c * nq + q) * ncol + j * lanes + l];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (mode == 1) s0 += t0[u] + t1[u], s1 += t2[u];
+            else if (lanes == 2) s0 += t0[u], s0 += t1[u];
+            else s0 += t0[u];
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
