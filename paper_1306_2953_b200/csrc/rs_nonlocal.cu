@@ -111,9 +111,11 @@ cudaError_t nl_launch(void (*kernel)(KArgs...), unsigned grid, unsigned block, s
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
-constexpr int NL_INFLIGHT = 8;     // points a thread of part 1 has in flight
-constexpr int NL_GPT = 4;          // points per thread in part 2
-constexpr int NL_LMG = 4;          // lm values reduced per pass through shared memory
+constexpr int NL_INFLIGHT = 4;     // points per thread in a unit of part 1
+constexpr int nl_cps(int lm) { return lm <= 4 ? 3 : lm <= 9 ? 2 : 1; }   // CTAs of part 1 per SM (registers: lm accumulators)
+constexpr int NL_GPT = 4;          // points per thread and batch in part 2
+constexpr int NL_GATHER_CPS = 3;   // persistent CTAs of part 2 per SM (80 registers; a 4th only fits with spills: slower)
+constexpr int NL_LMG = 2;          // lm values reduced per pass through shared memory
 
 __device__ __forceinline__ void cp_async8(void *dst_smem, const void *src)
 {
@@ -127,19 +129,23 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 constexpr int NL_STAGES = 3;
-constexpr size_t nl_project_smem(int vec, int nlm) { return (size_t)NL_STAGES * (NL_INFLIGHT * NL_THREADS * vec * 8 + NL_CHUNK * nlm * 8); }
+__host__ __device__ constexpr int nl_unit(int lshift) { return NL_INFLIGHT * (NL_THREADS >> lshift) < NL_CHUNK ? NL_INFLIGHT * (NL_THREADS >> lshift) : NL_CHUNK; }
+constexpr size_t nl_project_smem(int vec, int nlm, int lshift)
+{
+    return (size_t)NL_STAGES * (NL_INFLIGHT * NL_THREADS * vec * 8 + nl_unit(lshift) * nlm * 8);
+}
 
 // Part 1.  A thread owns VEC adjacent columns of the points prow, prow + rows, ... (L = ncol / VEC lanes per point,
 // rows = 256 / L points per pass) and LM accumulators per column.  The access chain item -> index -> psi row is three
 // dependent trips to memory, and a sphere is small (~17 chunks): one chunk per CTA leaves the machine waiting on
-// latency (measured: 1.9 TB/s).  So the CTAs are persistent (one per SM) and walk their chunks in UNITS of
-// min(256, 8 rows) points through a three-stage cp.async pipeline: while unit u is summed from shared memory the psi
+// latency (measured: 1.9 TB/s).  So the CTAs are persistent (one to three per SM) and walk their chunks in UNITS of
+// min(256, 4 rows) points through a three-stage cp.async pipeline: while unit u is summed from shared memory the psi
 // rows and projector values of units u+1 and u+2 are in flight and the indices of unit u+3 are being loaded.  A thread
 // reads back exactly the psi slots it copied; the projector values of a unit are one contiguous span copied by all.
 // Reduction over the points at the end of a chunk: shuffles inside a warp (when a warp holds several points), then
 // shared memory across the warps, both in a fixed order -> partial[item][lm][c].
 template <int VEC, int LM>
-__global__ void __launch_bounds__(NL_THREADS, 1) nl_project_kernel(const nl_item *__restrict__ items, int nitems, const int32_t *__restrict__ idx,
+__global__ void __launch_bounds__(NL_THREADS, nl_cps(LM)) nl_project_kernel(const nl_item *__restrict__ items, int nitems, const int32_t *__restrict__ idx,
                                                                   const double *__restrict__ gamma, int nlm, const double *__restrict__ psi,
                                                                   int ncol, int lshift, double *__restrict__ partial)
 {
@@ -149,8 +155,8 @@ __global__ void __launch_bounds__(NL_THREADS, 1) nl_project_kernel(const nl_item
     pdl_launch_dependents();
     const int tid = threadIdx.x, L = 1 << lshift, cl = tid & (L - 1), prow = tid >> lshift, rows = NL_THREADS >> lshift;
     const int c = cl * VEC;
-    const int sub = min(NL_CHUNK, NL_INFLIGHT * rows);                     // points per unit
-    const int psi_bytes = NL_INFLIGHT * NL_THREADS * VEC * 8, stage_bytes = psi_bytes + NL_CHUNK * nlm * 8;
+    const int sub = nl_unit(lshift);                                       // points per unit
+    const int psi_bytes = NL_INFLIGHT * NL_THREADS * VEC * 8, stage_bytes = psi_bytes + sub * nlm * 8;
     const int i0 = (int)((long long)blockIdx.x * nitems / gridDim.x), i1 = (int)((long long)(blockIdx.x + 1) * nitems / gridDim.x);
     struct unit {
         int item, q0, end, slot;                                          // points [q0, min(q0 + sub, end)) of the item; item < 0: none
@@ -272,39 +278,52 @@ __global__ void __launch_bounds__(128) nl_finalize_kernel(const int4 *__restrict
 // urec[u] = (mesh point, q of the first pair, its atom | (further pairs << 24), where the further pairs start in uext):
 // nearly every point lies in one sphere, so one 16-byte record starts all of a point's loads at once.
 template <int VEC, int LM>
-__global__ void __launch_bounds__(NL_THREADS) nl_gather_kernel(int nu, const int4 *__restrict__ urec, const int2 *__restrict__ uext,
+__global__ void __launch_bounds__(NL_THREADS, NL_GATHER_CPS) nl_gather_kernel(int nu, const int4 *__restrict__ urec, const int2 *__restrict__ uext,
                                                               const double *__restrict__ gamma, int nlm, const double *__restrict__ P,
                                                               double *__restrict__ hpsi, int ncol, int lshift)
 {
     using V = nl_vec<VEC>;
     const int tid = threadIdx.x, L = 1 << lshift, cl = tid & (L - 1), rows = NL_THREADS >> lshift;
     const int c = cl * VEC;
-    const int u0 = blockIdx.x * rows * NL_GPT + (tid >> lshift);
-    int4 rec[NL_GPT];
-    V h[NL_GPT];
+    const int per = rows * NL_GPT, nbatch = (nu + per - 1) / per;
+    auto load_rec = [&](int batch, int4 (&r)[NL_GPT]) {
+        const int u0 = batch * per + (tid >> lshift);
 #pragma unroll
-    for (int k = 0; k < NL_GPT; ++k) rec[k] = u0 + k * rows < nu ? urec[u0 + k * rows] : make_int4(-1, 0, 0, 0);
+        for (int k = 0; k < NL_GPT; ++k) r[k] = batch < nbatch && u0 + k * rows < nu ? urec[u0 + k * rows] : make_int4(-1, 0, 0, 0);
+    };
+    // persistent CTAs over batches of rows * NL_GPT points; the records of the next batch are loaded while the Hpsi rows
+    // of this one are in flight, so a batch costs one trip to memory, not two
+    int4 rec[NL_GPT], nxt[NL_GPT];
+    load_rec(blockIdx.x, rec);
+    bool waited = false;
+    for (int batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
+        V h[NL_GPT];
 #pragma unroll
-    for (int k = 0; k < NL_GPT; ++k) h[k] = rec[k].x >= 0 ? V::ld(hpsi + (size_t)rec[k].x * ncol + c) : V{};
-    pdl_wait();                                            // P of this call
+        for (int k = 0; k < NL_GPT; ++k) h[k] = rec[k].x >= 0 ? V::ld(hpsi + (size_t)rec[k].x * ncol + c) : V{};
+        load_rec(batch + gridDim.x, nxt);
+        if (!waited) pdl_wait(), waited = true;            // P of this call
 #pragma unroll
-    for (int k = 0; k < NL_GPT; ++k) {
-        if (rec[k].x < 0) continue;
-        const double *g = gamma + (size_t)rec[k].y * nlm;
-        const double *p = P + (size_t)(rec[k].z & 0xffffff) * nlm * ncol + c;   // 4-10 KB per atom: L1-resident
-        V s{};
+        for (int k = 0; k < NL_GPT; ++k) {
+            if (rec[k].x < 0) continue;
+            const double *g = gamma + (size_t)rec[k].y * nlm;
+            const double *p = P + (size_t)(rec[k].z & 0xffffff) * nlm * ncol + c;   // 4-10 KB per atom: L1-resident
+            V s{};
 #pragma unroll
-        for (int lm = 0; lm < LM; ++lm)
-            if (lm < nlm) s.fma_(g[lm], V::ld(p + (size_t)lm * ncol));
-        for (int e = rec[k].w, ee = e + (rec[k].z >> 24); e < ee; ++e) {
-            const int2 qa = uext[e];
-            g = gamma + (size_t)qa.x * nlm;
-            p = P + (size_t)qa.y * nlm * ncol + c;
-            for (int lm = 0; lm < nlm; ++lm) s.fma_(g[lm], V::ld(p + (size_t)lm * ncol));
+            for (int lm = 0; lm < LM; ++lm)
+                if (lm < nlm) s.fma_(g[lm], V::ld(p + (size_t)lm * ncol));
+            for (int e = rec[k].w, ee = e + (rec[k].z >> 24); e < ee; ++e) {
+                const int2 qa = uext[e];
+                g = gamma + (size_t)qa.x * nlm;
+                p = P + (size_t)qa.y * nlm * ncol + c;
+                for (int lm = 0; lm < nlm; ++lm) s.fma_(g[lm], V::ld(p + (size_t)lm * ncol));
+            }
+            h[k].add(s);
+            h[k].st(hpsi + (size_t)rec[k].x * ncol + c);
         }
-        h[k].add(s);
-        h[k].st(hpsi + (size_t)rec[k].x * ncol + c);
+#pragma unroll
+        for (int k = 0; k < NL_GPT; ++k) rec[k] = nxt[k];
     }
+    if (!waited) pdl_wait();
 }
 
 int ilog2n(int v)
@@ -477,7 +496,7 @@ extern "C" rs_status rs_nonlocal_prepare(rs_nonlocal *nl)
         // part 1 runs on persistent CTAs, CTA b taking the items [b n / G, (b + 1) n / G): consecutive items are mostly of
         // one atom, and a CTA reduces and stores a partial sum only where the atom changes or its range ends
         const int nitems = (int)nl->items.size();
-        nl->nctas = std::max(1, std::min(nitems, nl->m->sm_count > 0 ? nl->m->sm_count : 148));
+        nl->nctas = std::max(1, std::min(nitems, (nl->m->sm_count > 0 ? nl->m->sm_count : 148) * nl_cps(nl->nlm)));
         nl->nslots = 0;
         nl->atom_slots.clear();
         for (int b = 0; b < nl->nctas; ++b) {
@@ -493,7 +512,7 @@ extern "C" rs_status rs_nonlocal_prepare(rs_nonlocal *nl)
             }
         }
 #define NL_SMEM(VEC, LM) \
-    RS_CUDA_TRY(cudaFuncSetAttribute(nl_project_kernel<VEC, LM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nl_project_smem(VEC, LM)))
+    RS_CUDA_TRY(cudaFuncSetAttribute(nl_project_kernel<VEC, LM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nl_project_smem(VEC, LM, 0)))
         NL_SMEM(1, 4);
         NL_SMEM(1, 9);
         NL_SMEM(1, 16);
@@ -534,11 +553,11 @@ extern "C" rs_status rs_nonlocal_apply(rs_nonlocal *nl, const void *psi, void *h
     const double h3 = nl->m->h * nl->m->h * nl->m->h;
     const int vec = ncol >= 2 ? 2 : 1, lshift = ilog2n(ncol / vec);
     const int nu = (int)nl->urec.size(), per = (NL_THREADS >> lshift) * NL_GPT;
-    const unsigned g2 = (unsigned)((nu + per - 1) / per);
+    const unsigned g2 = (unsigned)std::min((nu + per - 1) / per, (nl->m->sm_count > 0 ? nl->m->sm_count : 148) * NL_GATHER_CPS);
     cudaError_t e1, e2, e3;
     const int nout = nl->nlm * ncol, nitems = (int)nl->items.size();
-    const unsigned g1 = (unsigned)nl->nctas;               // persistent, one CTA per SM
-    const size_t smem1 = nl_project_smem(vec, nl->nlm);
+    const unsigned g1 = (unsigned)nl->nctas;               // persistent
+    const size_t smem1 = nl_project_smem(vec, nl->nlm, lshift);
 #define NL_LAUNCH(VEC, LM)                                                                                                                \
     e1 = nl_launch(nl_project_kernel<VEC, LM>, g1, NL_THREADS, smem1, st, false, nl->d_items, nitems, nl->d_idx, nl->d_gamma, nl->nlm,       \
                    (const double *)psi, ncol, lshift, nl->d_partial);                                                                      \
