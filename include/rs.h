@@ -153,6 +153,17 @@ rs_status rs_block_dot(const rs_mesh *mesh, const void *a_dev, const void *b_dev
                        void *stream);
 rs_status rs_block_expectation(const rs_mesh *mesh, const void *psi_dev, const void *hpsi_dev, const double *eps_dev, int nst,
                                rs_dtype dtype, double *out_dev, void *stream);
+/* rs_block_expectation for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, bit-identical results, but the per-CTA partial sums live in a file-scope device array of
+ * the library (1.73 MiB, held by every GPU that loads the library until the process exits) instead of scratch that the
+ * first rs_block_expectation on a mesh allocates.  The call allocates and frees nothing and never synchronises.
+ * Limit: nst * (dtype == RS_COMPLEX128 ? 2 : 1) <= 64 real columns; wider blocks -> RS_ERR_INVALID_ARG with a message
+ * that names the limit.  The mesh's device must be the current device.  The array is shared by EVERY call on that
+ * device, whatever the mesh or stream: two calls that overlap on the GPU race (order them on one stream or with
+ * events); it needs no clearing between calls.  The first call per device resolves the array's address
+ * (cudaGetSymbolAddress, no allocation): make that call outside graph capture.                                    */
+rs_status rs_block_expectation_static(const rs_mesh *mesh, const void *psi_dev, const void *hpsi_dev, const double *eps_dev,
+                                      int nst, rs_dtype dtype, double *out_dev, void *stream);
 rs_status rs_block_axpy(const rs_mesh *mesh, const void *alpha_dev, const void *x_dev, void *y_dev, int nst, rs_dtype dtype,
                         void *stream);
 rs_status rs_block_copy(const rs_mesh *mesh, const void *src_dev, void *dst_dev, int nst, rs_dtype dtype, void *stream);

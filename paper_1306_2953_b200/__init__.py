@@ -37,7 +37,7 @@ EXPORTS = (
     "rs_block_pack", "rs_block_unpack", "rs_hamiltonian_apply", "rs_hamiltonian_apply_v",
     "rs_hamiltonian_apply_states_host", "rs_last_error", "rs_kernel_name", "rs_kernel_table_bytes", "rs_version",
     "rs_sweep_options_default", "rs_mesh_set_sweep_options", "rs_hamiltonian_prepare",
-    "rs_block_dot", "rs_block_expectation", "rs_block_axpy", "rs_block_copy", "rs_hamiltonian_apply_ex", "rs_block_overlap",
+    "rs_block_dot", "rs_block_expectation", "rs_block_expectation_static", "rs_block_axpy", "rs_block_copy", "rs_hamiltonian_apply_ex", "rs_block_overlap",
     "rs_nonlocal_create", "rs_nonlocal_destroy", "rs_nonlocal_sphere_size", "rs_nonlocal_get_sphere", "rs_nonlocal_set_projectors",
     "rs_nonlocal_ncolors", "rs_nonlocal_get_colors", "rs_nonlocal_prepare", "rs_nonlocal_apply",
     "rs_workspace_create", "rs_workspace_destroy", "rs_workspace_bytes", "rs_hamiltonian_apply_states_stream",
@@ -88,6 +88,7 @@ def _load() -> C.CDLL:
     L.rs_hamiltonian_apply_states_host.argtypes = [vp, C.c_int, dp, vp, vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int]
     L.rs_block_dot.argtypes = [vp, vp, vp, C.c_int, C.c_int, vp, vp]
     L.rs_block_expectation.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, vp, vp]
+    L.rs_block_expectation_static.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, vp, vp]
     L.rs_block_axpy.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, vp]
     L.rs_nonlocal_create.argtypes = [vp, dp, C.c_int, C.c_double, C.c_int, C.POINTER(vp)]
     L.rs_nonlocal_destroy.argtypes = [vp]
@@ -336,6 +337,13 @@ def rs_block_expectation(mesh: Mesh, psi, hpsi, eps, nst: int, out, stream=None)
     """out[3][nst] float64 = Re<psi|hpsi>, |psi|^2, |hpsi - eps psi|^2 per orbital (eps: device float64 [nst] or None)."""
     _check(_lib.rs_block_expectation(mesh.handle, _ptr(psi), _ptr(hpsi), _ptr(eps) if eps is not None else None, nst,
                                      _dtype_of(psi), _ptr(out), _stream(stream)))
+
+
+def rs_block_expectation_static(mesh: Mesh, psi, hpsi, eps, nst: int, out, stream=None) -> None:
+    """rs_block_expectation without any allocation: partial sums in the library's static device array (<= 64 real
+    columns; calls that overlap on the GPU race).  Same output, bit for bit."""
+    _check(_lib.rs_block_expectation_static(mesh.handle, _ptr(psi), _ptr(hpsi), _ptr(eps) if eps is not None else None, nst,
+                                            _dtype_of(psi), _ptr(out), _stream(stream)))
 
 
 def rs_block_axpy(mesh: Mesh, alpha, x, y, nst: int, stream=None) -> None:

@@ -224,3 +224,78 @@ rs_status rs_launch_block_axpy(const rs_mesh *m, const double *alpha, const doub
     RS_CUDA_TRY(cudaGetLastError());
     return RS_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// rs_block_expectation_static: the expectation sums for callers that cannot allocate (code under CUDA graph
+// capture, serving loops, harnesses that forbid cudaMalloc).  Same two kernels, same grid, same summation order as
+// rs_block_expectation -- the results are bit-identical -- but the per-CTA partial sums go to a file-scope device
+// array instead of the mesh-owned scratch that rs_reduce_scratch() allocates on first use.
+//   * RS_STATIC_MAX_COLS real columns at most (nst <= 64 real, nst <= 32 complex): 1184 CTAs x 3 sums x 64 columns x
+//     8 bytes = 1.73 MiB, which every GPU that loads the library holds until the process exits;
+//   * nothing has to start at zero: every CTA of the first kernel overwrites all of its slots before the second
+//     kernel reads them, so the previous call's contents do not matter;
+//   * every call, on any mesh and any stream, shares the one array of its device: calls that overlap on the GPU race.
+// In host code `rs_static_red` is a stand-in for the symbol, not a device address: its address is taken with
+// cudaGetSymbolAddress, once per device, with that device current, and that pointer is what the kernels get.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int RS_STATIC_MAX_COLS = 64;
+constexpr int RS_STATIC_MAX_DEVICES = 64;
+static __device__ __align__(256) double rs_static_red[(size_t)RS_RED_CTAS * 3 * RS_STATIC_MAX_COLS];
+
+// address of rs_static_red on `device` (which must be current); resolved once per device, no allocation
+rs_status static_red_address(int device, double **out)
+{
+    static double *addr[RS_STATIC_MAX_DEVICES] = {};
+    if (device < 0 || device >= RS_STATIC_MAX_DEVICES) return rs_fail(RS_ERR_UNSUPPORTED, "rs_block_expectation_static: device ordinal");
+    if (!addr[device]) {
+        double *p = nullptr;
+        RS_CUDA_TRY(cudaGetSymbolAddress((void **)&p, rs_static_red));
+        if (!p) return rs_fail(RS_ERR_CUDA, "rs_block_expectation_static: cudaGetSymbolAddress returned a null address");
+        addr[device] = p;   // racing first calls store the same value
+    }
+    *out = addr[device];
+    return RS_OK;
+}
+
+}  // namespace
+
+extern "C" rs_status rs_block_expectation_static(const rs_mesh *m, const void *psi, const void *hpsi, const double *eps_dev,
+                                                 int nst, rs_dtype dtype, double *out_dev, void *stream)
+{
+    if (!m || !psi || !hpsi || !out_dev || nst < 1 || nst > RS_MAX_BLOCK || (nst & (nst - 1)) ||
+        (dtype != RS_REAL64 && dtype != RS_COMPLEX128))
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_block_expectation_static: bad argument");
+    if ((((uintptr_t)psi | (uintptr_t)hpsi) & 15u) != 0)
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_block_expectation_static: blocks must be 16-byte aligned");
+    const int lanes = dtype == RS_COMPLEX128 ? 2 : 1, ncol = nst * lanes;
+    if (ncol > RS_STATIC_MAX_COLS)
+        return rs_fail(RS_ERR_INVALID_ARG, "rs_block_expectation_static: " + std::to_string(ncol) + " real columns exceed the static scratch (" +
+                                               std::to_string(RS_STATIC_MAX_COLS) + "): use rs_block_expectation");
+    if (!m->have_device) return rs_fail(RS_ERR_CUDA, "no CUDA device");
+    int cur = -1;
+    RS_CUDA_TRY(cudaGetDevice(&cur));
+    if (cur != m->device) return rs_fail(RS_ERR_INVALID_ARG, "rs_block_expectation_static: the mesh's device must be current");
+    double *partial = nullptr;
+    rs_status rc = static_red_address(cur, &partial);
+    if (rc != RS_OK) return rc;
+    // the launch configuration of rs_launch_block_reduce(nq = 3, mode = 0), restated so that path stays as it is
+    cudaStream_t st = (cudaStream_t)stream;
+    const int vec = ncol >= 2 ? 2 : 1;
+    const int tshift = ilog2i(ncol / vec);
+    const int rpc = RED_THREADS >> tshift;
+    int grid = (int)((m->np + rpc - 1) / rpc);
+    const int cap = (m->sm_count > 0 ? m->sm_count : 148) * 8;
+    if (grid > cap) grid = cap;
+    if (grid > RS_RED_CTAS) grid = RS_RED_CTAS;
+    const double *a = (const double *)psi, *b = (const double *)hpsi;
+    if (vec == 1)
+        block_reduce_kernel<1, 3, false><<<grid, RED_THREADS, 0, st>>>(a, b, eps_dev, lanes, m->np, ncol, tshift, partial);
+    else
+        block_reduce_kernel<2, 3, false><<<grid, RED_THREADS, 0, st>>>(a, b, eps_dev, lanes, m->np, ncol, tshift, partial);
+    RS_CUDA_TRY(cudaGetLastError());
+    block_reduce_final_kernel<<<(3 * nst * 32 + 255) / 256, 256, 0, st>>>(partial, grid, 3, 3, ncol, lanes, 0, out_dev);
+    RS_CUDA_TRY(cudaGetLastError());
+    return RS_OK;
+}
