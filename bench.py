@@ -412,6 +412,15 @@ def main() -> None:
                 "apply_share_of_step": apply_ms * nblocks / ms_step,
                 "apply_gflops": B * npts * flops_per_output(n) * conv / (apply_ms * 1e-3) / 1e9,
                 "apply_gflops_executed": B * npts * flops_per_output(n) * lanes / (apply_ms * 1e-3) / 1e9}
+    # second bound of the same kernel: plain fp64 arithmetic (DFMA issues at one warp instruction
+    # per 2 clocks per scheduler = 64 lanes per SM; peak = SMs x 64 x 2 flops x the SM clock sampled during this run)
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sm_mhz = float((clocks or {}).get("sm_mhz") or 0.0) or 1965.0
+    alu_peak = sm_count * 64 * 2 * sm_mhz * 1e6 / 1e12
+    roofline["alu"] = {"bound": "alu", "achieved": roofline["apply_gflops_executed"] / 1e3, "peak": alu_peak, "unit": "TFLOP/s",
+                       "frac": roofline["apply_gflops_executed"] / 1e3 / alu_peak,
+                       "note": "useful flops only (2(6n+1)+2 per output); the kernel also spends fp64 issue slots on points of "
+                               "partly filled tiles and on the 2n centre-only planes around every work piece"}
     traffic = traffic_rows()
     row = traffic.get(f"config{cfg.index}_B{B}_n{n}_{kname}")
     if row:    # from a committed ncu capture of this kernel, not from this run
