@@ -35,6 +35,7 @@ struct ov_shape {
     static constexpr int STAGES = 3;
     static constexpr int CPS = C <= 16 ? 3 : C <= 64 ? 2 : 1;
     static constexpr int PITCH = C % 16 == 0 ? C + 4 : C == 8 ? 12 : 4; // doubles; = 4 or 12 (mod 16)
+    static constexpr bool PAIRED = MT % 2 == 0 && NT % 2 == 0;   // 16-byte fragment loads (64 columns: 0.62 -> 0.56 ms)
     static constexpr int TILE = P * PITCH;                              // doubles per operand per stage
     static constexpr size_t SMEM_RING = (size_t)STAGES * 2 * TILE * 8;
     static constexpr size_t SMEM_RED = (size_t)KS * C * C * 8;
@@ -110,10 +111,25 @@ __global__ void __launch_bounds__(OV_THREADS, S::CPS) overlap_kernel(const doubl
         for (int kk = 0; kk < KSTEPS; ++kk) {
             const int prow = (ks * KSTEPS + kk) * 4 + (lane & 3);
             double af[S::MT], bf[S::NT];
+            if constexpr (S::PAIRED) {
+                // one 16-byte load feeds two tiles: tile 2q takes the even, tile 2q + 1 the odd columns of a 16-column group
+                // (the output indices below undo the interleave); quarter-warps stay bank-conflict free (pitch / 2 = 2 mod 8)
 #pragma unroll
-            for (int i = 0; i < S::MT; ++i) af[i] = xs[prow * PITCH + (wm * S::MT + i) * 8 + (lane >> 2)];
+                for (int i = 0; i < S::MT; i += 2) {
+                    const double2 t = *reinterpret_cast<const double2 *>(xs + prow * PITCH + (wm * S::MT + i) * 8 + 2 * (lane >> 2));
+                    af[i] = t.x, af[i + 1] = t.y;
+                }
 #pragma unroll
-            for (int j = 0; j < S::NT; ++j) bf[j] = ys[prow * PITCH + (wn * S::NT + j) * 8 + (lane >> 2)];
+                for (int j = 0; j < S::NT; j += 2) {
+                    const double2 t = *reinterpret_cast<const double2 *>(ys + prow * PITCH + (wn * S::NT + j) * 8 + 2 * (lane >> 2));
+                    bf[j] = t.x, bf[j + 1] = t.y;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < S::MT; ++i) af[i] = xs[prow * PITCH + (wm * S::MT + i) * 8 + (lane >> 2)];
+#pragma unroll
+                for (int j = 0; j < S::NT; ++j) bf[j] = ys[prow * PITCH + (wn * S::NT + j) * 8 + (lane >> 2)];
+            }
 #pragma unroll
             for (int i = 0; i < S::MT; ++i)
 #pragma unroll
@@ -129,9 +145,14 @@ __global__ void __launch_bounds__(OV_THREADS, S::CPS) overlap_kernel(const doubl
     for (int i = 0; i < S::MT; ++i)
 #pragma unroll
         for (int j = 0; j < S::NT; ++j) {
-            const int row = (wm * S::MT + i) * 8 + (lane >> 2), col = (wn * S::NT + j) * 8 + 2 * (lane & 3);
+            int row = (wm * S::MT + i) * 8 + (lane >> 2), col = (wn * S::NT + j) * 8 + 2 * (lane & 3), col1 = col + 1;
+            if constexpr (S::PAIRED) {
+                row = (wm * S::MT + (i & ~1)) * 8 + 2 * (lane >> 2) + (i & 1);
+                col = (wn * S::NT + (j & ~1)) * 8 + 4 * (lane & 3) + (j & 1);
+                col1 = col + 2;
+            }
             red[((size_t)ks * C + row) * C + col] = acc[i][j][0];
-            red[((size_t)ks * C + row) * C + col + 1] = acc[i][j][1];
+            red[((size_t)ks * C + row) * C + col1] = acc[i][j][1];
         }
     __syncthreads();
     for (int e = tid; e < C * C; e += OV_THREADS) {
