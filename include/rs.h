@@ -30,7 +30,7 @@
  *     (a cudaStream_t passed as void*; NULL = legacy default stream).  After
  *     rs_hamiltonian_prepare(mesh, fd_order, nst, dtype) they allocate nothing and never synchronise.
  *     Without it, the first apply of a given (fd_order, block width) prepares lazily (host table build, one
- *     synchronous cudaMalloc + copy, cached in the handle); blocks wider than 16 real columns also encode
+ *     synchronous cudaMalloc + copy, cached in the handle); blocks of 8 or more than 16 real columns also encode
  *     their tensor maps once per psi buffer address (host-only work, cached).
  *   - Alignment: vloc 8 bytes; states 8 (real) / 16 (complex) bytes; block buffers (psi, hpsi) 16 bytes
  *     (bulk copies and vector accesses) -> RS_ERR_INVALID_ARG otherwise.

@@ -49,8 +49,13 @@ static rs_kernel resolve_kernel(const rs_mesh *m, int n, int ncol, rs_kernel k)
 {
     // below ~1 M outputs the persistent kernel's start-up (tables, pipeline fill: ~20 us) outweighs its streaming rate
     // (measured: config 0 x 16 columns, gather 0.028 ms vs sweep 0.051 ms; config 1 x 16, 0.055 vs 0.051)
-    if (k == RS_KERNEL_AUTO)
-        return (m->np * (int64_t)ncol >= (1 << 20) && rs_sweep_usable(m, n, ncol)) ? RS_KERNEL_SWEEP : RS_KERNEL_GATHER;
+    // 8 columns run as half a 16-column slice (the plane-sweep kernel does the work of 16): worth it only on large meshes
+    // (measured: config 1, 0.25 M points: gather 0.025 ms vs sweep 0.033-0.040; config 2, 1.96 M points: 0.148 vs 0.139-0.148;
+    // config 4, 3.8 M points: 0.284 vs 0.234-0.256, fd_order 6: 0.430 vs 0.298-0.348)
+    if (k == RS_KERNEL_AUTO) {
+        const int64_t outputs = m->np * (int64_t)ncol, least = ncol < 16 ? ((int64_t)1 << 23) + ((int64_t)1 << 22) : ((int64_t)1 << 20);
+        return (outputs >= least && rs_sweep_usable(m, n, ncol)) ? RS_KERNEL_SWEEP : RS_KERNEL_GATHER;
+    }
     return k;
 }
 

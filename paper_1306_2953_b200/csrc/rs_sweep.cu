@@ -427,7 +427,7 @@ __device__ __forceinline__ void tm_wait_row(uint32_t (&r)[N * 8])
     tm_wait_ld32(lo);
 }
 
-template <class S>
+template <class S, bool HALF>
 __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_weights &w, const unsigned char *smem,
                                                uint32_t full0, uint32_t empty0, uint32_t tmem_base, int nsteps, int tid,
                                                long long *step_clock)
@@ -474,6 +474,12 @@ __device__ __forceinline__ void sweep_consumer(const sweep_args &a, const rs_wei
             for (int j = 0; j < PY; ++j) {
                 const uint4 q = *reinterpret_cast<const uint4 *>(sp + irow + j * 64);
                 io[4 * j] = q.x, io[4 * j + 1] = q.y, io[4 * j + 2] = q.z, io[4 * j + 3] = q.w;
+            }
+            if constexpr (HALF) {   // 8-column block: the upper lanes hold the zero-filled columns and own no output
+                if (c >= SW_C / 2) {
+#pragma unroll
+                    for (int q = 0; q < PY * PZ; ++q) io[q] = 0xffffffffu;
+                }
             }
 
             if (mode == MODE_FULL) {
@@ -596,7 +602,7 @@ __device__ __forceinline__ void setmaxnreg_dec()
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(REGS));
 }
 
-template <class S, bool TENSOR>
+template <class S, bool TENSOR, bool HALF = false>
 __global__ void __launch_bounds__(S::THREADS, 1)
 sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_weights w, const __grid_constant__ sweep_maps maps)
 {
@@ -643,7 +649,7 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
                                   a.recs + (size_t)item.x * S::REC_BYTES, nsteps, ptid, 3.0 * w.w[0]);
     } else {
         setmaxnreg_inc<S::CONS_REGS>();
-        sweep_consumer<S>(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid,
+        sweep_consumer<S, HALF>(a, w, smem, smem_u32(&full_bar[0]), smem_u32(&empty_bar[0]), tmem_base_s, nsteps, ctid,
                           a.step_clock ? a.step_clock + item.x : nullptr);
         named_bar_sync(1, S::CONSUMERS);
         if (ctid == 0 && a.cycles) a.cycles[blockIdx.x] = clock64() - clock0;
@@ -659,6 +665,12 @@ sweep_kernel(const __grid_constant__ sweep_args a, const __grid_constant__ rs_we
 // ---------------------------------------------------------------------------------------------
 namespace {
 enum { VARIANT_N4 = 0, VARIANT_N6 = 1, VARIANT_NONE = -1 };
+// Block widths (real columns): multiples of 16 are processed 16 columns at a time; 8 columns run as HALF a slice -- the
+// tensor-map boxes are 16 columns wide whatever the block's width, the copy unit zero-fills the 8 columns that lie
+// outside the row, and the consumer lanes of those columns compute on zeros and store nothing.
+constexpr int SW_HALF = SW_C / 2;
+bool sweep_width_ok(int ncol) { return ncol == SW_HALF || (ncol >= SW_C && ncol % SW_C == 0); }
+int sweep_nchunks(int ncol) { return ncol < SW_C ? 1 : ncol / SW_C; }
 int sweep_variant(int n) { return n == 4 ? VARIANT_N4 : n == 6 ? VARIANT_N6 : VARIANT_NONE; }
 shape_rt variant_shape(int variant) { return variant == VARIANT_N6 ? shape_of<shape_n6>() : shape_of<shape_n4>(); }
 }  // namespace
@@ -713,11 +725,11 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
                          const rs_sweep_costs *measured, const std::vector<std::vector<rs_sweep_piece>> *given_pieces)
 {
     const int variant = sweep_variant(n);
-    if (variant == VARIANT_NONE || ncol % SW_C != 0 || nctas < 1) return false;
+    if (variant == VARIANT_NONE || !sweep_width_ok(ncol) || nctas < 1) return false;
     const shape_rt sh = variant_shape(variant);
     const int N = sh.N, TY = sh.TY, TZ = SW_TZ, WY = sh.WY, WZ = sh.WZ;
     tile_geometry g{m, sh, m->dims[0], m->dims[1], m->dims[2], (m->dims[1] + TY - 1) / TY, (m->dims[2] + TZ - 1) / TZ};
-    const int nx = g.nx, nchunks = ncol / SW_C;
+    const int nx = g.nx, nchunks = sweep_nchunks(ncol);
     out = rs_sweep_host();
     out.rec_bytes = sh.rec_bytes;
 
@@ -952,7 +964,7 @@ bool rs_sweep_build_host(const rs_mesh *m, int n, int ncol, int max_planes, int 
 
 bool rs_sweep_supported(const rs_mesh *m, int n, int ncol)
 {
-    return m->ordering == RS_ORDER_LEX && !m->periodic && sweep_variant(n) != VARIANT_NONE && ncol >= SW_C && ncol % SW_C == 0 &&
+    return m->ordering == RS_ORDER_LEX && !m->periodic && sweep_variant(n) != VARIANT_NONE && sweep_width_ok(ncol) &&
            (uint64_t)(m->np + 1) * (uint64_t)ncol < 0xffffffffull;   // store offsets are 32-bit element offsets
 }
 
@@ -964,13 +976,17 @@ static cudaError_t set_smem()
 {
     cudaError_t e = cudaFuncSetAttribute(sweep_kernel<S, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sweep_kernel<S, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
+    if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(sweep_kernel<S, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
 }
 
 template <class S>
 static void launch_shape(bool tensor, unsigned grid, cudaStream_t st, const sweep_args &a, const rs_weights &w, const sweep_maps &maps)
 {
-    if (tensor)
+    if (a.ncol == (uint32_t)SW_HALF)
+        sweep_kernel<S, true, true><<<grid, S::THREADS, S::SMEM, st>>>(a, w, maps);
+    else if (tensor)
         sweep_kernel<S, true><<<grid, S::THREADS, S::SMEM, st>>>(a, w, maps);
     else
         sweep_kernel<S, false><<<grid, S::THREADS, S::SMEM, st>>>(a, w, maps);
@@ -1146,8 +1162,12 @@ const char *rs_sweep_variant_name(const rs_mesh *m, int n, int ncol)
 {
     const bool tensor = ncol != SW_C || m->opt.force_tensor;
     switch (sweep_variant(n)) {
-        case VARIANT_N6: return tensor ? "sweep[n6 c16 8x16 q2p4 persistent ws tma2d+tmem s3]" : "sweep[n6 c16 8x16 q2p4 persistent ws tma1d+tmem s3]";
-        default: return tensor ? "sweep[n4 c16 16x16 q4p4 persistent ws tma2d+tmem s3]" : "sweep[n4 c16 16x16 q4p4 persistent ws tma1d+tmem s3]";
+        case VARIANT_N6:
+            if (ncol == SW_HALF) return "sweep[n6 c8-in-16 8x16 q2p4 persistent ws tma2d+tmem s3]";
+            return tensor ? "sweep[n6 c16 8x16 q2p4 persistent ws tma2d+tmem s3]" : "sweep[n6 c16 8x16 q2p4 persistent ws tma1d+tmem s3]";
+        default:
+            if (ncol == SW_HALF) return "sweep[n4 c8-in-16 16x16 q4p4 persistent ws tma2d+tmem s3]";
+            return tensor ? "sweep[n4 c16 16x16 q4p4 persistent ws tma2d+tmem s3]" : "sweep[n4 c16 16x16 q4p4 persistent ws tma1d+tmem s3]";
     }
 }
 
@@ -1181,7 +1201,7 @@ std::string rs_sweep_selfcheck_host(const rs_mesh *m, int n, int ncol, int max_p
         const int32_t v = map[(size_t)ip * NS + axis * 2 * N + 2 * (std::abs(k) - 1) + (k > 0 ? 0 : 1)];
         return v == np ? -1 : v;
     };
-    const int nchunks = ncol / SW_C;
+    const int nchunks = sweep_nchunks(ncol);
     std::vector<uint8_t> done((size_t)np * nchunks, 0);
     int64_t npieces = 0;
     auto fail = [&](int cta, int step, const char *what, int y, int z, int k) {

@@ -136,10 +136,11 @@ def test_autotune_keeps_parity():
     assert st[:, 4].sum() > 0 and (st[:, 4] <= 8 * st[:, 1]).all() and len(set(st[:, 4].tolist())) > 1
 
 
-@pytest.mark.parametrize("seed,n,B", [(0, 4, 16), (1, 4, 32), (2, 6, 16), (3, 6, 32)])
+@pytest.mark.parametrize("seed,n,B", [(0, 4, 16), (1, 4, 32), (2, 6, 16), (3, 6, 32), (4, 4, 8), (5, 6, 8)])
 def test_sweep_kernel_ragged_clusters(seed, n, B):
     """Small spheres scattered so that z-rows break into several copy runs of odd lengths and most tiles are nearly
-    empty: 1-D bulk copies (B = 16) and overlapping 2-D tensor boxes (B = 32), before and after the autotuned re-deal."""
+    empty: 1-D bulk copies (B = 16), overlapping 2-D tensor boxes (B = 32) and boxes wider than the block's rows
+    (B = 8: half a slice, the copy unit zero-fills the other half), before and after the autotuned re-deal."""
     rng = np.random.default_rng(seed)
     nc = int(rng.integers(4, 12))
     centers = rng.uniform(0.0, 9.0, (nc, 3))
@@ -373,25 +374,26 @@ def test_kernel_choice_is_reported():
 # oracle (the oracle does a whole orbital of these meshes in a fraction of a second per core).
 @pytest.mark.parametrize("B", [1, 2, 4, 8, 16, 32, 64])
 def test_config2_full_mesh_block(B):
-    """Every block size BASELINE.json configs[2] names, on the full 1.96 M-point mesh (B < 16: the gather kernel)."""
+    """Every block size BASELINE.json configs[2] names, on the full 1.96 M-point mesh (B = 8: half a 16-column slice of the
+    plane-sweep kernel; B < 8: the gather kernel)."""
     p = problem(2)
     cfg = p.cfg
     nst = B + 3 if B == 16 else B                       # B = 16: a second, ragged block as well
     psi = synthetic.orbitals(cfg.seed, 0, nst, p.np)
     g = _run(p, psi, 4, B, "auto")
-    assert rs.rs_kernel_name(p.mesh, 4, B).startswith("sweep[" if B >= 16 else "gather")
+    assert rs.rs_kernel_name(p.mesh, 4, B).startswith("sweep[" if B >= 8 else "gather")
     o = p.oracle_hpsi(psi, 4, nthreads=16)
     check(g, o, p.cond_denominator(psi, 4), f"config2 B={B}")
 
 
 @pytest.mark.parametrize("B", [1, 2, 4, 8, 16, 32])
 def test_config3_complex_full_mesh_block(B):
-    """Every block size BASELINE.json configs[3] names (complex: 2 B real columns; B < 8: the gather kernel)."""
+    """Every block size BASELINE.json configs[3] names (complex: 2 B real columns; B < 4: the gather kernel)."""
     p = problem(2)                                       # config 3 = config 2's mesh and potential, complex orbitals
     cfg = synthetic.config(3)
     psi = synthetic.orbitals(cfg.seed, 0, B, p.np, is_complex=True)
     g = _run(p, psi, 4, B, "auto")
-    assert rs.rs_kernel_name(p.mesh, 4, B, rs.RS_COMPLEX128).startswith("sweep[" if B >= 8 else "gather")
+    assert rs.rs_kernel_name(p.mesh, 4, B, rs.RS_COMPLEX128).startswith("sweep[" if B >= 4 else "gather")
     o = p.oracle_hpsi(psi, 4, nthreads=16)
     check(g, o, p.cond_denominator(psi, 4), f"config3 complex B={B}")
 

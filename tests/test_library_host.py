@@ -268,8 +268,10 @@ def test_sweep_selfcheck_on_boxes_and_unsupported_calls():
     assert e.value.status == rs.RS_ERR_UNSUPPORTED
     mesh = rs.rs_mesh_create_box(8, 8, 8, 0.25, 5, False, rs.RS_ORDER_LEX)
     with pytest.raises(rs.RsError) as e:
-        rs.rs_sweep_selfcheck(mesh, 4, 8)                                           # 8 real columns: gather kernel only
+        rs.rs_sweep_selfcheck(mesh, 4, 4)                                           # 4 real columns: gather kernel only
     assert e.value.status == rs.RS_ERR_UNSUPPORTED
+    rs.rs_sweep_selfcheck(mesh, 4, 8)                                               # 8 real columns: half a 16-column slice
+    rs.rs_sweep_selfcheck(mesh, 4, 4, rs.RS_COMPLEX128)
     with pytest.raises(rs.RsError) as e:
         rs.rs_sweep_selfcheck(mesh, 5, 16)                                          # fd_order 5: gather kernel only
     assert e.value.status == rs.RS_ERR_UNSUPPORTED
