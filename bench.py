@@ -472,6 +472,13 @@ def main() -> None:
                           "alg_gbs": ab / ms / 1e6, "frac_measured": ab / ms / 1e6 / peak, "frac_of_8TBs": ab / ms / 1e6 / 8000.0,
                           "traffic": (int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])) if row else None,
                           "note": "block working set may fit L2" if 2 * b1.numel() * b1.element_size() < 126e6 else ""})
+            if kn.startswith("sweep[") and Bs * lanes < 16 and kern == rs.RS_KERNEL_AUTO:
+                # 8 columns run as half a 16-column slice of the plane-sweep kernel (it does the work of 16 columns, and its
+                # compact records make the algorithmic byte count smaller than the gather kernel's): the alternative beside it
+                msg = time_apply(rs, torch, mesh, n, coeffs, v, b1, b2, Bs, rs.RS_KERNEL_GATHER, reps)
+                abg = algorithmic_bytes(npts, Bs * lanes, rs.rs_kernel_table_bytes(mesh, n, Bs, rsdt, rs.RS_KERNEL_GATHER))
+                sweep[-1].update({"gather_apply_ms": msg, "gather_alg_gbs": abg / msg / 1e6, "gather_frac_measured": abg / msg / 1e6 / peak,
+                                  "note": "half slice of the sweep kernel: faster than the gather kernel, fewer algorithmic bytes"})
             del b1, b2
 
     # ---- the operations around H psi on the same block: time and algorithmic rates -------
