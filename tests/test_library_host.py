@@ -350,6 +350,12 @@ def test_next_row_entry_points_check_arguments_without_a_device():
     c = np.array([-205 / 72, 8 / 5, -1 / 5, 8 / 315, -1 / 560])
     assert L.rs_hamiltonian_apply_ex(h, 4, c.ctypes.data_as(C.POINTER(C.c_double)), ptr(out), ptr(a), ptr(b), 4, rs.RS_REAL64, None,
                                      None, None) == rs.RS_ERR_INVALID_ARG
+    # the allocation-free expectation sums: 64 real columns at most, whatever the device
+    wide = aligned((npts + 1) * 128)
+    assert L.rs_block_expectation_static(h, ptr(wide), ptr(wide), None, 64, rs.RS_COMPLEX128, ptr(out), None) == rs.RS_ERR_INVALID_ARG
+    assert b"static scratch" in L.rs_last_error()
+    assert L.rs_block_expectation_static(h, ptr(a[1:]), ptr(b), None, 4, rs.RS_REAL64, ptr(out), None) == rs.RS_ERR_INVALID_ARG
+    assert L.rs_block_expectation_static(h, ptr(a), ptr(b), None, 3, rs.RS_REAL64, ptr(out), None) == rs.RS_ERR_INVALID_ARG
     nl0 = rs.rs_nonlocal_create(m, np.zeros((1, 3)), 0.6, 1)
     nl0.set_projectors(0, np.ones((nl0.sphere(0).size, 1)))
     assert L.rs_nonlocal_apply(nl0._h, ptr(a[1:]), ptr(b), 4, rs.RS_REAL64, None) == rs.RS_ERR_INVALID_ARG      # misaligned block
@@ -357,6 +363,7 @@ def test_next_row_entry_points_check_arguments_without_a_device():
     import torch
     if not torch.cuda.is_available():
         for call in (lambda: L.rs_block_dot(h, ptr(a), ptr(b), 4, rs.RS_REAL64, ptr(out), None),
+                     lambda: L.rs_block_expectation_static(h, ptr(a), ptr(b), None, 4, rs.RS_REAL64, ptr(out), None),
                      lambda: L.rs_block_overlap(h, ptr(a), ptr(b), 4, rs.RS_REAL64, ptr(out), None),
                      lambda: L.rs_block_axpy(h, ptr(out), ptr(a), ptr(b), 4, rs.RS_REAL64, None),
                      lambda: L.rs_block_copy(h, ptr(a), ptr(b), 4, rs.RS_REAL64, None),
